@@ -1,0 +1,213 @@
+/*
+ * nms.h -- C ABI of the B200-native direct-summation SANS core
+ * (data-parallel hot path of arxiv/paper_2601_18444, "NuMagSANS").
+ *
+ * Citations "Lnnn"/"Eq. n" refer to /root/reference/PAPER.md; "reading n" to
+ * DESIGN.md section 3.  Everything behind this header is hand-written CUDA for
+ * sm_100a in paper_2601_18444_b200/csrc/; there is no CPU fallback: without a
+ * CUDA device nms_create() fails with NMS_E_CUDA.
+ *
+ * General conventions
+ *  - Pointers are tagged [dev] (device memory, caller-owned, e.g. a torch tensor's
+ *    data_ptr()) or [host].  The library never frees or keeps a caller pointer:
+ *    nms_set_sample() copies what it needs into context-owned device storage.
+ *  - Every call only ENQUEUES work on the context's CUDA stream (given to
+ *    nms_create; 0 = legacy default stream).  Results are valid after
+ *    nms_synchronize() or a stream synchronisation by the caller.  The *_host
+ *    entry point is the exception: it synchronises before returning.
+ *  - Errors: return code + nms_last_error(); no exceptions, no abort, no stdout.
+ *    Argument errors are detected before any launch and leave the context usable.
+ *  - Units: positions nm, q nm^-1 (L393), r nm (L404); only q.r must be dimensionless.
+ *  - Geometry (Fig. 1 L33, Eq. 6): beam along x, detector in the y-z plane,
+ *    q = (0, q_y, q_z) = q (0, sin th, cos th), th measured from +z towards +y.
+ *  - Amplitude planes, in this order: Re N~, Im N~, Re M~x, Im M~x, Re M~y, Im M~y,
+ *    Re M~z, Im M~z; they are the RAW sums of Eq. 42-47 (L353-L368) without the
+ *    (2 pi)^-3/2 or (W N)^-1/2 prefactors (reading 4); the imaginary parts carry the
+ *    minus sign of e^{-i q.r} (Eq. 45, 47).
+ */
+#ifndef NMS_H_
+#define NMS_H_
+
+#include <stdint.h>
+
+#if defined(__GNUC__)
+#define NMS_API __attribute__((visibility("default")))
+#else
+#define NMS_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct nms_ctx nms_ctx;
+
+typedef enum {
+    NMS_OK = 0,
+    NMS_E_ARG = 1,          /* bad argument (NULL, non-positive size, unknown kind, non-orthonormal R, ...) */
+    NMS_E_STATE = 2,        /* call order violated (e.g. nms_response before nms_amplitudes) */
+    NMS_E_CUDA = 3,         /* CUDA runtime error or no usable device; text in nms_last_error() */
+    NMS_E_NOMEM = 4,        /* host or device allocation failed */
+    NMS_E_UNSUPPORTED = 5
+} nms_status;
+
+/* The 13 base response functions of Section II (L35-L174), all real, per detector point.
+ * With N = sN N~, M = sM M~, q^ = (0, sin th, cos th), Q = q^ x (q^ x M) (Eq. 5, Eq. 7),
+ * Pi = P.Q, every kind is multiplied by invV (see nms_set_scales):                              */
+typedef enum {
+    NMS_NUC = 0,        /* |N|^2                         Eq. 3  L48  */
+    NMS_MAG = 1,        /* |Q|^2                         Eq. 4  L50  */
+    NMS_UNPOL = 2,      /* NUC + MAG = (PP+MM+PM+MP)/2   Eq. 27-28 */
+    NMS_PROJ = 3,       /* |Pi|^2                        Eq. 8  L66  */
+    NMS_NM = 4,         /* P.(N Q* + N* Q) = 2 Re(N Pi*) Eq. 18 */
+    NMS_SF = 5,         /* MAG - PROJ                    Eq. 13  */
+    NMS_CHI = 6,        /* -i P.(Q x Q*)                 Eq. 14  */
+    NMS_PM = 7,         /* (+-) = SF + CHI               Eq. 11  */
+    NMS_MP = 8,         /* (-+) = SF - CHI               Eq. 12  */
+    NMS_PP = 9,         /* (++) = NUC + NM + PROJ        Eq. 16 */
+    NMS_MM = 10,        /* (--) = NUC - NM + PROJ        Eq. 17 */
+    NMS_POL_PLUS = 11,  /* (+) = PP + PM                 Eq. 23 */
+    NMS_POL_MINUS = 12, /* (-) = MM + MP                 Eq. 24 */
+    NMS_KIND_COUNT = 13
+} nms_kind;
+
+/* Detector grid.  The abscissa arrays are HOST arrays (they are tiny and the library analyses
+ * them on the host to pick the kernel variant); they are copied during the call.
+ *  type 0 polar     : u0 = |q| [n0], u1 = theta [n1] (radians); q_y = q sin th, q_z = q cos th (L343),
+ *                     evaluated in fp64 from the float values.
+ *  type 1 cartesian : u0 = q_z [n0], u1 = q_y [n1]; theta = atan2(q_y, q_z), theta(0,0) = 0 (reading 5).
+ *  type 2 list      : u0 = q_y [n0], u1 = q_z [n0], n1 must be 1; theta as for cartesian.
+ * Flat detector index = i0 * n1 + i1 (i1 fastest); n_q = n0 * n1.                                 */
+typedef struct {
+    int type;
+    int n0, n1;
+    const float* u0;   /* [host] */
+    const float* u1;   /* [host] */
+} nms_qgrid;
+
+/* Kernels whose device time nms_kernel_time_ms() can report (CUDA events on the context stream). */
+typedef enum {
+    NMS_T_PREP = 0,         /* a-1 rotate + pack                                    */
+    NMS_T_AMPLITUDE = 1,    /* a-2 direct sums (also the a-6 per-particle variant)  */
+    NMS_T_EPILOGUE = 2,     /* a-3 reduce + responses                               */
+    NMS_T_AZIMUTHAL = 3,    /* a-4                                                  */
+    NMS_T_CORRELATION = 4,  /* a-5                                                  */
+    NMS_T_COUNT = 5
+} nms_timer;
+
+/* ---- context ---------------------------------------------------------------------------------- */
+
+/* Create a context on CUDA device `device` that enqueues on `cuda_stream` (a cudaStream_t cast to
+ * void*; NULL = default stream).  Fails with NMS_E_CUDA if no device is usable or the device is not
+ * compute capability 10.x.  *out is NULL on failure.                                              */
+NMS_API nms_status nms_create(nms_ctx** out, int device, void* cuda_stream);
+/* Synchronise the stream and free everything the context owns.  NULL is allowed. */
+NMS_API void nms_destroy(nms_ctx* ctx);
+/* Text of the last error on this context ("" if none).  Valid until the next call on the context. */
+NMS_API const char* nms_last_error(const nms_ctx* ctx);
+/* Block until all work enqueued by this context has finished. */
+NMS_API nms_status nms_synchronize(nms_ctx* ctx);
+
+/* ---- sample (a-1, Eq. 37-41) --------------------------------------------------------- */
+
+/* Define the real-space sample: W cells with positions pos [dev][W][3] (x,y,z), nuclear weights
+ * N [dev][W] or NULL (nuclear channel absent, N~ = 0) and moments m [dev][W][3] or NULL (magnetic
+ * channel absent) -- the activation switches of L242.  R [host][9] is the row-major sample rotation
+ * (Eq. 37), NULL = identity; it must be orthonormal within 1e-6 (else NMS_E_ARG).  Positions AND
+ * moments are rotated (reading 2): r' = R (x + r^k), m' = R m, in fp64, rounded once.  The arrays are
+ * copied; they may be released once the stream has passed this call.  Resets particles to "none". */
+NMS_API nms_status nms_set_sample(nms_ctx* ctx, const float* pos, const float* N, const float* m, int64_t W,
+                          const double* R);
+/* Optional object structure (L310-L317): offsets [host][K+1], offsets[0] = 0, non-decreasing,
+ * offsets[K] = W; cells of object k are [offsets[k], offsets[k+1]).  centres [dev][K][3] are the
+ * StructData positions r^k added to the local coordinates before rotation (Eq. 38-40), or NULL
+ * (r^k = 0, L341).  K = 0 removes the structure.  Needed by nms_form_factor_split.              */
+NMS_API nms_status nms_set_particles(nms_ctx* ctx, const int64_t* offsets, int64_t K, const float* centres);
+/* Change the rotation only (rocking scans): re-runs the prep pass on the stored sample. */
+NMS_API nms_status nms_set_rotation(nms_ctx* ctx, const double* R);
+/* Polarisation direction P [host][3] (L64, L272); normalised on input; default (0,0,1). */
+NMS_API nms_status nms_set_polarization(nms_ctx* ctx, const double* P);
+/* Scale factors (reading 4): N = sN N~, M = sM M~, every response is multiplied by invV.  Defaults 1.
+ * Absolute units of the paper: sN = N_s V_cell, sM = b_H M_s V_cell, invV = 1/V (Eq. 48).   */
+NMS_API nms_status nms_set_scales(nms_ctx* ctx, double sN, double sM, double invV);
+
+/* ---- amplitudes and responses (a-2, a-3) -------------------------------------------------------- */
+
+/* Direct sums A_c(q) = sum_j w_cj exp(-i q.r'_j) for every detector point (Eq. 42-47).  The result
+ * is kept in the context (fp64) for nms_response; if out_amp [dev][8][n_q] (float) is not NULL the
+ * eight planes are also written there.  The grid becomes the context's current grid.             */
+NMS_API nms_status nms_amplitudes(nms_ctx* ctx, const nms_qgrid* grid, float* out_amp);
+/* Response maps out [dev][n_kinds][n_q] (float) from the amplitudes of the last nms_amplitudes call
+ * (NMS_E_STATE if there was none since the last sample change).                                  */
+NMS_API nms_status nms_response(nms_ctx* ctx, const nms_kind* kinds, int n_kinds, float* out);
+/* Fused a-2 + a-3: amplitudes and all requested responses without materialising the amplitudes.
+ * This is the call bench.py times.  out [dev][n_kinds][n_q] (float).                             */
+NMS_API nms_status nms_compute(nms_ctx* ctx, const nms_qgrid* grid, const nms_kind* kinds, int n_kinds, float* out);
+
+/* ---- azimuthal average (a-4, Eq. 30) ------------------------------------------------------ */
+
+/* Average maps [dev][n_maps][n_q] (float) over the azimuth on the context's current grid.
+ *  - polar grid and q_hi <= q_lo: n_bins must equal n0; bin i is ring i, value = arithmetic mean
+ *    over theta (periodic trapezoid, reading 7), abscissa q_i, count n1.
+ *  - otherwise: n_bins uniform bins on [q_lo, q_hi): bin = floor((|q|-q_lo)/(q_hi-q_lo)*n_bins) in
+ *    fp64 exactly in this order with |q| = sqrt(q_y^2+q_z^2); points outside are dropped; value =
+ *    mean of the members; empty bins give 0 with count 0; abscissa = bin centre (reading 8).
+ * out_I [dev][n_maps][n_bins] (float); out_q [dev][n_bins] (float) or NULL; out_count
+ * [dev][n_bins] (int32) or NULL.                                                                 */
+NMS_API nms_status nms_azimuthal_average(nms_ctx* ctx, const float* maps, int n_maps, int n_bins, double q_lo,
+                                 double q_hi, float* out_I, float* out_q, int32_t* out_count);
+
+/* ---- correlation function (a-5, Eq. 34-35) -------------------------------------------- */
+
+/* c(r_k) = (1/2pi^2) trapz_q[ I(q) j0(q r_k) q^2 ], p(r_k) = r_k^2 c(r_k), for each of n_maps curves
+ * I [dev][n_maps][n_bins] (float) on abscissae q_of_bin [dev][n_bins] (float, ascending).  Bins whose
+ * count [dev][n_bins] (int32) is 0 are skipped (count NULL = none skipped); the trapezoid runs over the
+ * remaining abscissae only, no extrapolation (reading 9); j0(x) = 1 - x^2/6 for |x| < 1e-4.  Arithmetic
+ * in fp64.  r [dev][n_r] (float); out_c, out_p [dev][n_maps][n_r] (float).                       */
+NMS_API nms_status nms_correlation(nms_ctx* ctx, const float* I, const float* q_of_bin, const int32_t* count,
+                           int n_maps, int n_bins, const float* r, int n_r, float* out_c, float* out_p);
+
+/* ---- form factor / interference split (a-6, Eq. 49-50) -------------------------------- */
+
+/* For every requested kind B: out_total = B(sum_p A_p, sum_p A_p), out_form = sum_p B(A_p, A_p), where
+ * A_p are the amplitudes of object p alone (with its centre); interference = total - form (reading 13).
+ * Needs nms_set_particles (NMS_E_STATE otherwise).  Each output [dev][n_kinds][n_q] (float); either
+ * may be NULL.                                                                                   */
+NMS_API nms_status nms_form_factor_split(nms_ctx* ctx, const nms_qgrid* grid, const nms_kind* kinds, int n_kinds,
+                                 float* out_total, float* out_form);
+
+/* ---- end-to-end host entry point ---------------------------------------------------------------- */
+
+/* One whole step from HOST buffers: copy pos/N/m [host] to the device, prep, amplitudes + responses,
+ * optional azimuthal average and correlation, copy the results back to HOST buffers and synchronise.
+ * out_maps [host][n_kinds][n_q] (float) or NULL.  If n_bins > 0: out_I [host][n_kinds][n_bins], and if
+ * additionally n_r > 0 (r [host][n_r]): out_c, out_p [host][n_kinds][n_r].  Pinned host memory makes
+ * the copies asynchronous; pageable memory also works.                                           */
+NMS_API nms_status nms_run_host(nms_ctx* ctx, const float* pos, const float* N, const float* m, int64_t W,
+                        const double* R, const nms_qgrid* grid, const nms_kind* kinds, int n_kinds,
+                        float* out_maps, int n_bins, double q_lo, double q_hi, float* out_I,
+                        const float* r, int n_r, float* out_c, float* out_p);
+
+/* ---- introspection / tuning --------------------------------------------------------------------- */
+
+/* sum_j |w_cj| of the rotated weights, c = N, m'x, m'y, m'z, into out [host][4] (the denominators of
+ * the amplitude tolerance 1e-5 sum|w|); synchronises.                                            */
+NMS_API nms_status nms_get_weight_sums(nms_ctx* ctx, double* out);
+
+/* Integer options.  "variant": 0 auto, 1 force the direct (MUFU per pair) kernel, 2 force the
+ * recurrence kernel (NMS_E_UNSUPPORTED at compute time if the detector lines are not equally spaced).
+ * "timing": 1 records CUDA events around each kernel.  "chunks": 0 auto, else the number of cell
+ * chunks.  "qt": 0 auto, else detector points per thread (4, 8 or 16).  Unknown keys: NMS_E_ARG. */
+NMS_API nms_status nms_set_option(nms_ctx* ctx, const char* key, int64_t value);
+/* Read back integers: "launches" (kernels launched by this context so far), "variant_used" (1 general
+ * direct, 2 polar direct, 4 cartesian direct, 3 line recurrence), "n_chunks", "n_tiles", "n_slots",
+ * "sm_count", "blocks_per_sm", "qt".                                                             */
+NMS_API nms_status nms_get_info(nms_ctx* ctx, const char* key, int64_t* value);
+/* Device time in ms of the most recent launch of the given kernel class ("timing" must be 1);
+ * synchronises on that kernel's end event.  NMS_E_STATE if it has not run.                       */
+NMS_API nms_status nms_kernel_time_ms(nms_ctx* ctx, nms_timer which, float* ms);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NMS_H_ */

@@ -1,0 +1,197 @@
+// k_prep.cu -- a-1: rotate + pack the real-space sample into tiles, and detector set-up.
+//
+//  prep kernel   (Eq. 37-41):  r' = R (x + r^k), m' = R m in fp64; only Y, Z (rows 2, 3 of R)
+//                are kept because q_x = 0 on the detector (Eq. 41).  One block per tile: it finds the
+//                tile's bounding-box midpoint (Y0, Z0), stores cells relative to it (one rounding to
+//                fp32) and accumulates sum_j |w_cj| for the tolerance denominators.
+//  qsetup kernel (Eq. 6): per detector point (q_y, q_z) in fp64 [rad/nm] and
+//                (sin th, cos th) for the response epilogue.
+#include "nms_internal.h"
+
+namespace nms {
+
+constexpr int PREP_THREADS = 256;
+constexpr int PREP_PER_THREAD = TILE / PREP_THREADS;
+
+struct PrepArgs {
+    const float* pos;
+    const float* N;
+    const float* m;
+    const float* centres;
+    const TileSrc* src;
+    const int64_t* first_slot;
+    const int32_t* flags;
+    TileMeta* meta;
+    float4* A;
+    float2* B;
+    double* wsum;
+    double R[9];
+};
+
+__device__ __forceinline__ double warp_min(double v)
+{
+    for (int o = 16; o > 0; o >>= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+__device__ __forceinline__ double warp_max(double v)
+{
+    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+__device__ __forceinline__ double warp_sum(double v)
+{
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+__global__ void __launch_bounds__(PREP_THREADS) k_prep(const PrepArgs a)
+{
+    __shared__ double red[8][PREP_THREADS / 32];
+    __shared__ double origin[2];
+    const int tile = blockIdx.x;
+    const TileSrc ts = a.src[tile];
+    const int64_t first_slot = a.first_slot[tile];
+    const int n_slots = (ts.n_src + SLOT_PAD - 1) / SLOT_PAD * SLOT_PAD;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+
+    double cx = 0.0, cy = 0.0, cz = 0.0;
+    if (a.centres && ts.particle >= 0) {
+        cx = (double)a.centres[3 * (int64_t)ts.particle + 0];
+        cy = (double)a.centres[3 * (int64_t)ts.particle + 1];
+        cz = (double)a.centres[3 * (int64_t)ts.particle + 2];
+    }
+    double Y[PREP_PER_THREAD], Z[PREP_PER_THREAD];
+    float wN[PREP_PER_THREAD], wx[PREP_PER_THREAD], wy[PREP_PER_THREAD], wz[PREP_PER_THREAD];
+    double ymin = INFINITY, ymax = -INFINITY, zmin = INFINITY, zmax = -INFINITY;
+    double sN = 0.0, sx = 0.0, sy = 0.0, sz = 0.0;
+#pragma unroll
+    for (int u = 0; u < PREP_PER_THREAD; ++u) {
+        const int i = tid + u * PREP_THREADS;
+        Y[u] = Z[u] = 0.0;
+        wN[u] = wx[u] = wy[u] = wz[u] = 0.f;
+        if (i < ts.n_src) {
+            const int64_t j = ts.src_first + i;
+            const double x = (double)a.pos[3 * j + 0] + cx;
+            const double y = (double)a.pos[3 * j + 1] + cy;
+            const double z = (double)a.pos[3 * j + 2] + cz;
+            Y[u] = a.R[3] * x + a.R[4] * y + a.R[5] * z;   // Eq. 39
+            Z[u] = a.R[6] * x + a.R[7] * y + a.R[8] * z;   // Eq. 40
+            ymin = fmin(ymin, Y[u]); ymax = fmax(ymax, Y[u]);
+            zmin = fmin(zmin, Z[u]); zmax = fmax(zmax, Z[u]);
+            if (a.N) { wN[u] = a.N[j]; sN += fabs((double)wN[u]); }
+            if (a.m) {
+                const double mx = (double)a.m[3 * j + 0], my = (double)a.m[3 * j + 1], mz = (double)a.m[3 * j + 2];
+                const double rx = a.R[0] * mx + a.R[1] * my + a.R[2] * mz;   // m' = R m (reading 2)
+                const double ry = a.R[3] * mx + a.R[4] * my + a.R[5] * mz;
+                const double rz = a.R[6] * mx + a.R[7] * my + a.R[8] * mz;
+                sx += fabs(rx); sy += fabs(ry); sz += fabs(rz);
+                wx[u] = (float)rx; wy[u] = (float)ry; wz[u] = (float)rz;
+            }
+        }
+    }
+    ymin = warp_min(ymin); ymax = warp_max(ymax); zmin = warp_min(zmin); zmax = warp_max(zmax);
+    sN = warp_sum(sN); sx = warp_sum(sx); sy = warp_sum(sy); sz = warp_sum(sz);
+    if (lane == 0) {
+        red[0][warp] = ymin; red[1][warp] = ymax; red[2][warp] = zmin; red[3][warp] = zmax;
+        red[4][warp] = sN; red[5][warp] = sx; red[6][warp] = sy; red[7][warp] = sz;
+    }
+    __syncthreads();
+    if (tid == 0) {
+        double v[8];
+        for (int r = 0; r < 8; ++r) v[r] = red[r][0];
+        for (int w = 1; w < PREP_THREADS / 32; ++w) {
+            v[0] = fmin(v[0], red[0][w]); v[1] = fmax(v[1], red[1][w]);
+            v[2] = fmin(v[2], red[2][w]); v[3] = fmax(v[3], red[3][w]);
+            for (int r = 4; r < 8; ++r) v[r] += red[r][w];
+        }
+        const double Y0 = ts.n_src > 0 ? 0.5 * (v[0] + v[1]) : 0.0;
+        const double Z0 = ts.n_src > 0 ? 0.5 * (v[2] + v[3]) : 0.0;
+        origin[0] = Y0; origin[1] = Z0;
+        TileMeta tm;
+        tm.Y0 = Y0; tm.Z0 = Z0; tm.first_slot = first_slot; tm.n_slots = n_slots; tm.flags = a.flags[tile];
+        a.meta[tile] = tm;
+        for (int r = 0; r < 4; ++r)
+            if (v[4 + r] != 0.0) atomicAdd(a.wsum + r, v[4 + r]);
+    }
+    __syncthreads();
+    const double Y0 = origin[0], Z0 = origin[1];
+#pragma unroll
+    for (int u = 0; u < PREP_PER_THREAD; ++u) {
+        const int i = tid + u * PREP_THREADS;
+        if (i < n_slots) {
+            float4 va; float2 vb;
+            if (i < ts.n_src) {
+                va = make_float4((float)(Y[u] - Y0), (float)(Z[u] - Z0), wN[u], wx[u]);
+                vb = make_float2(wy[u], wz[u]);
+            } else {
+                va = make_float4(0.f, 0.f, 0.f, 0.f);
+                vb = make_float2(0.f, 0.f);
+            }
+            a.A[first_slot + i] = va;
+            a.B[first_slot + i] = vb;
+        }
+    }
+}
+
+nms_status launch_prep(nms_ctx* c)
+{
+    PrepArgs a;
+    a.pos = (const float*)c->raw_pos.p;
+    a.N = c->has_N ? (const float*)c->raw_N.p : nullptr;
+    a.m = c->has_M ? (const float*)c->raw_m.p : nullptr;
+    a.centres = c->has_centres ? (const float*)c->centres.p : nullptr;
+    a.src = (const TileSrc*)c->tile_src.p;
+    // first_slot and flags live behind the TileSrc array in the same buffer (see build_tiles in nms_api.cu)
+    const char* base = (const char*)c->tile_src.p + sizeof(TileSrc) * (size_t)c->n_tiles;
+    a.first_slot = (const int64_t*)base;
+    a.flags = (const int32_t*)(base + sizeof(int64_t) * (size_t)c->n_tiles);
+    a.meta = (TileMeta*)c->tile_meta.p;
+    a.A = (float4*)c->cellA.p;
+    a.B = (float2*)c->cellB.p;
+    a.wsum = (double*)c->wsum.p;
+    for (int i = 0; i < 9; ++i) a.R[i] = c->R[i];
+    NMS_CUDA(c, cudaMemsetAsync(c->wsum.p, 0, 4 * sizeof(double), c->stream));
+    timer_begin(c, NMS_T_PREP);
+    k_prep<<<(unsigned)c->n_tiles, PREP_THREADS, 0, c->stream>>>(a);
+    timer_end(c, NMS_T_PREP);
+    c->launches += 1;
+    NMS_CUDA(c, cudaGetLastError());
+    return NMS_OK;
+}
+
+// ---- detector set-up ---------------------------------------------------------------------------
+__global__ void k_qsetup(int type, int n0, int n1, const float* __restrict__ u0, const float* __restrict__ u1,
+                         double2* __restrict__ qc, double2* __restrict__ sc)
+{
+    const int64_t f = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t nq = (int64_t)n0 * n1;
+    if (f >= nq) return;
+    const int i0 = (int)(f / n1), i1 = (int)(f % n1);
+    double qy, qz, s, c;
+    if (type == 0) {                       // polar: q_y = q sin th, q_z = q cos th (L343)
+        const double q = (double)u0[i0], th = (double)u1[i1];
+        sincos(th, &s, &c);
+        qy = q * s; qz = q * c;
+    } else {
+        if (type == 1) { qz = (double)u0[i0]; qy = (double)u1[i1]; }
+        else           { qy = (double)u0[i0]; qz = (double)u1[i0]; }
+        const double n = sqrt(qy * qy + qz * qz);
+        if (n > 0.0) { s = qy / n; c = qz / n; }     // th = atan2(q_y, q_z)
+        else         { s = 0.0; c = 1.0; }           // th(0,0) = 0 (reading 5)
+    }
+    qc[f] = make_double2(qy, qz);
+    sc[f] = make_double2(s, c);
+}
+
+nms_status launch_qsetup(nms_ctx* c)
+{
+    const int threads = 256;
+    const unsigned blocks = (unsigned)((c->n_q + threads - 1) / threads);
+    k_qsetup<<<blocks, threads, 0, c->stream>>>(c->g_type, c->g_n0, c->g_n1, (const float*)c->u0.p,
+                                                (const float*)c->u1.p, (double2*)c->qc.p, (double2*)c->sc.p);
+    c->launches += 1;
+    NMS_CUDA(c, cudaGetLastError());
+    return NMS_OK;
+}
+
+}  // namespace nms

@@ -1,0 +1,140 @@
+// nms_internal.h -- shared declarations of the CUDA implementation behind include/nms.h.
+// Nothing here is part of the ABI.  Citations "Lnnn"/"Eq. n" refer to PAPER.md (see include/nms.h).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <vector>
+#include "../../include/nms.h"
+
+namespace nms {
+
+// ---- packed real-space layout (a-1) ----------------------------------------------------------
+// Cells are grouped into tiles of at most TILE consecutive cells (never straddling an object when
+// an object structure is set).  Each tile carries a local origin (Y0,Z0) in fp64; a cell stores its
+// rotated detector-plane coordinates RELATIVE to that origin (Eq. 39-40 minus origin) and its
+// weights:  A[slot] = (dY, dZ, N, m'x),  B[slot] = (m'y, m'z).   X is never needed: q_x = 0 (Eq. 41).
+// Tiles are padded to a multiple of 8 slots with zero-weight cells so that every bulk copy is
+// 16-byte aligned and the inner loop can be unrolled without a tail.
+constexpr int TILE = 1024;
+constexpr int SLOT_PAD = 8;
+
+struct TileMeta {          // consumed by the amplitude kernel
+    double Y0, Z0;         // local origin [nm]
+    int64_t first_slot;    // index into A/B
+    int32_t n_slots;       // padded cell count (multiple of SLOT_PAD)
+    int32_t flags;         // bit 0: last tile of its object (form-factor split)
+};
+struct TileSrc {           // consumed by the prep kernel
+    int64_t src_first;     // first source cell
+    int32_t n_src;         // number of source cells (<= TILE)
+    int32_t particle;      // object index (for centres), -1 if none
+};
+
+struct Timer {
+    cudaEvent_t beg = nullptr, end = nullptr;
+    bool ran = false;
+};
+
+struct DevBuf {
+    void* p = nullptr;
+    size_t cap = 0;
+};
+
+}  // namespace nms
+
+struct nms_ctx {
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    int sm_count = 0;
+    char err[512] = {0};
+
+    // options
+    int opt_variant = 0;   // 0 auto, 1 direct, 2 recurrence
+    int opt_timing = 0;
+    int opt_chunks = 0;
+    int opt_qt = 0;        // 0 auto, else 4/8/16
+    int64_t launches = 0;
+    int variant_used = 0, n_chunks_used = 0, blocks_per_sm_used = 0, qt_used = 0;
+
+    // sample (raw copy kept for nms_set_rotation)
+    int64_t W = 0;
+    bool has_N = false, has_M = false;
+    nms::DevBuf raw_pos, raw_N, raw_m, centres;
+    std::vector<int64_t> offsets;      // host, K+1 entries (empty = no object structure)
+    int64_t K = 0;
+    bool has_centres = false;
+    double R[9] = {1, 0, 0, 0, 1, 0, 0, 0, 1};
+    double P[3] = {0, 0, 1};
+    double sN = 1.0, sM = 1.0, invV = 1.0;
+
+    // packed sample
+    bool packed_valid = false;
+    int64_t n_tiles = 0, n_slots = 0;
+    std::vector<nms::TileSrc> h_tile_src;
+    std::vector<int32_t> h_tile_flags;
+    std::vector<int64_t> h_tile_first_slot;
+    nms::DevBuf tile_src, tile_meta, cellA, cellB, wsum;   // wsum: double[4]
+
+    // current detector grid
+    bool grid_valid = false;
+    int g_type = 0, g_n0 = 0, g_n1 = 0;
+    int64_t n_q = 0;
+    bool g_uniform = false;            // abscissa along the thread line (u0) is equally spaced
+    std::vector<float> h_u0, h_u1;
+    nms::DevBuf u0, u1, qc, sc;        // qc: double2[n_q] (q_y,q_z) rad/nm; sc: double2[n_q] (sin th, cos th)
+
+    // amplitudes / scratch
+    bool amp_valid = false;
+    nms::DevBuf amp64;                 // double [8][n_q]
+    nms::DevBuf part, ppart, formpart; // chunk partials
+    nms::DevBuf chunk_begin;           // int32 [n_chunks+1] (split mode only)
+    std::vector<int32_t> h_chunk_begin;
+    nms::DevBuf kinds_dev;             // int32 [<=13]
+    nms::DevBuf bin_idx, bin_sum, bin_cnt;
+    nms::DevBuf host_stage[8];         // device staging for nms_run_host
+
+    nms::Timer timers[NMS_T_COUNT];
+};
+
+namespace nms {
+
+nms_status fail(nms_ctx* c, nms_status st, const char* fmt, ...);
+nms_status cuda_fail(nms_ctx* c, cudaError_t e, const char* where);
+nms_status ensure(nms_ctx* c, DevBuf& b, size_t bytes);
+void timer_begin(nms_ctx* c, int which);
+void timer_end(nms_ctx* c, int which);
+
+#define NMS_CUDA(c, call)                                          \
+    do {                                                           \
+        cudaError_t e__ = (call);                                  \
+        if (e__ != cudaSuccess) return nms::cuda_fail((c), e__, #call); \
+    } while (0)
+
+// ---- kernel launchers (each only enqueues on c->stream) ----------------------------------------
+// k_prep.cu
+nms_status launch_prep(nms_ctx* c);                       // a-1: raw sample -> packed tiles, wsum
+nms_status launch_qsetup(nms_ctx* c);                     // detector abscissae -> qc, sc
+// k_amplitude.cu
+struct AmpPlan {
+    int variant;       // 1 general direct, 2 line direct, 3 line recurrence
+    int qt;            // q points per thread
+    int n_chunks;
+    int n_qblocks;
+    int blocks_per_sm;
+    bool split;
+};
+nms_status plan_amplitude(nms_ctx* c, bool split, AmpPlan* plan);
+nms_status launch_amplitude(nms_ctx* c, const AmpPlan& plan, const int32_t* kinds_dev, int n_kinds);
+// k_epilogue.cu
+nms_status launch_epilogue(nms_ctx* c, int n_chunks, const int32_t* kinds_dev, int n_kinds, float* out_maps,
+                           float* out_amp, bool keep_amp64);
+nms_status launch_response_from_amp(nms_ctx* c, const int32_t* kinds_dev, int n_kinds, float* out_maps);
+nms_status launch_split_epilogue(nms_ctx* c, int n_chunks, const int32_t* kinds_dev, int n_kinds, float* out_total,
+                                 float* out_form);
+// k_post.cu
+nms_status launch_azimuthal(nms_ctx* c, const float* maps, int n_maps, int n_bins, double q_lo, double q_hi,
+                            float* out_I, float* out_q, int32_t* out_count);
+nms_status launch_correlation(nms_ctx* c, const float* I, const float* q_of_bin, const int32_t* count, int n_maps,
+                              int n_bins, const float* r, int n_r, float* out_c, float* out_p);
+
+}  // namespace nms

@@ -1,0 +1,392 @@
+"""GPU-vs-oracle parity of the hot path (run on the B200 box: pytest -m gpu).
+
+Every test calls the CUDA path through the C ABI (via the same-name Python binding) and compares it
+with the fp64 oracle on the same seeded inputs.  Tolerances are the ones BASELINE.json's north_star
+states: each amplitude within 1e-5 * sum_j |w_j| of the oracle, each cross section within relative
+1e-3 wherever it exceeds 1e-6 of its maximum.
+"""
+import numpy as np
+import pytest
+
+import nms_inputs as ni
+from nms_inputs import KIND_INDEX as KI
+
+pytestmark = pytest.mark.gpu
+
+AMP_TOL = 1e-5      # x sum_j |w_cj|
+XS_RTOL = 1e-3      # relative, where |oracle| > XS_FLOOR * max|oracle|
+XS_FLOOR = 1e-6
+
+
+@pytest.fixture(scope="module")
+def nms():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    import paper_2601_18444_b200 as mod
+    return mod
+
+
+@pytest.fixture()
+def ctx(nms):
+    c = nms.Context(0)
+    yield c.h
+    c.close()
+
+
+def _t(a, dtype=None):
+    import torch
+    if a is None:
+        return None
+    return torch.as_tensor(np.ascontiguousarray(a), device="cuda") if dtype is None else torch.as_tensor(np.ascontiguousarray(a, dtype=dtype), device="cuda")
+
+
+def _upload(nms, h, wl, R=None):
+    pos, N, m = _t(wl.pos), _t(wl.N), _t(wl.m)
+    nms.nms_set_sample(h, pos, N, m, wl.R if R is None else R)
+    if wl.offsets is not None:
+        nms.nms_set_particles(h, wl.offsets, _t(wl.centres))
+    nms.nms_set_polarization(h, wl.P)
+    return pos, N, m
+
+
+def assert_amplitudes(A_gpu, A_ref, wsum, label=""):
+    """|A_gpu - A_ref| <= 1e-5 sum|w_c| per component; exactly zero where the component has no weight."""
+    for c in range(4):
+        for part in (0, 1):
+            d = np.abs(A_gpu[2 * c + part].astype(np.float64) - A_ref[2 * c + part])
+            if wsum[c] == 0.0:
+                assert np.all(A_gpu[2 * c + part] == 0.0), f"{label}: component {c} must be exactly zero"
+            else:
+                worst = d.max() / wsum[c]
+                assert worst <= AMP_TOL, f"{label}: amplitude plane {2 * c + part}: max err {worst:.3e} x sum|w|"
+
+
+def assert_cross_sections(M_gpu, M_ref, kinds, label="", ref_max=None):
+    for i, k in enumerate(kinds):
+        ref = M_ref[i]
+        mx = np.abs(ref).max() if ref_max is None else ref_max[i]
+        sel = np.abs(ref) > XS_FLOOR * mx
+        if not np.any(sel):
+            continue
+        rel = np.abs(M_gpu[i].astype(np.float64)[sel] - ref[sel]) / np.abs(ref[sel])
+        assert rel.max() <= XS_RTOL, f"{label}: kind {ni.KINDS[k]}: max rel err {rel.max():.3e} at {sel.sum()} points"
+
+
+def _oracle_maps(oracle_mod, wl, qy, qz, th, kinds, R=None):
+    A, wsum = oracle_mod.amplitudes(wl.pos, wl.N, wl.m, wl.R if R is None else R, qy, qz, offsets=wl.offsets,
+                                    centres=wl.centres, return_wsum=True)
+    M = oracle_mod.response(A, th, kinds, P=wl.P)
+    return A, wsum, M
+
+
+def _run_full(nms, h, wl, kinds):
+    import torch
+    nq = wl.grid.n_q
+    amp = torch.empty((8, nq), dtype=torch.float32, device="cuda")
+    maps = torch.empty((len(kinds), nq), dtype=torch.float32, device="cuda")
+    maps2 = torch.empty_like(maps)
+    nms.nms_amplitudes(h, wl.grid, amp)
+    nms.nms_response(h, kinds, maps)
+    nms.nms_compute(h, wl.grid, kinds, maps2)
+    nms.nms_synchronize(h)
+    assert torch.equal(maps, maps2), "nms_compute and nms_amplitudes+nms_response disagree"
+    return amp.cpu().numpy(), maps.cpu().numpy()
+
+
+# ---------------------------------------------------------------------------------------------------
+# C1, C2 at full size, full maps; every kernel variant the grid admits
+# ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name", ["C1", "C2"])
+@pytest.mark.parametrize("variant,qt", [(0, 0), (1, 0), (2, 8), (2, 16), (1, 4), (2, 4)])
+def test_full_config_maps(nms, ctx, oracle_mod, name, variant, qt):
+    wl = ni.make_config(name)
+    kinds = list(ni.ALL_KINDS)
+    _upload(nms, ctx, wl)
+    nms.nms_set_option(ctx, "variant", variant)
+    nms.nms_set_option(ctx, "qt", qt)
+    A_gpu, M_gpu = _run_full(nms, ctx, wl, kinds)
+    qy, qz, th = oracle_mod.grid_points(wl.grid)
+    A, wsum, M = _oracle_maps(oracle_mod, wl, qy, qz, th, kinds)
+    np.testing.assert_allclose(nms.nms_get_weight_sums(ctx), wsum, rtol=1e-12)
+    assert_amplitudes(A_gpu, A, wsum, name)
+    assert_cross_sections(M_gpu, M, kinds, name)
+    used = nms.nms_get_info(ctx, "variant_used")
+    assert used == (3 if variant != 1 else (2 if wl.grid.type == 0 else 4))
+
+
+def test_c1_physics_on_gpu(nms, ctx):
+    """Uniform M_z sphere (Eq. 60-63): MAG = |F|^2 sin^2 th, SF = |F|^2 sin^2 cos^2, CHI = 0 exactly."""
+    wl = ni.make_config("C1")
+    _upload(nms, ctx, wl)
+    kinds = [KI["NUC"], KI["MAG"], KI["SF"], KI["CHI"]]
+    _, M = _run_full(nms, ctx, wl, kinds)
+    th = np.tile(wl.grid.u1.astype(np.float64), wl.grid.n0)
+    s2, c2 = np.sin(th) ** 2, np.cos(th) ** 2
+    big = M[0] > 1e-6 * M[0].max()
+    np.testing.assert_allclose(M[1][big], (M[0] * s2)[big], rtol=2e-6, atol=1e-6 * M[0].max() * 1e-6)
+    np.testing.assert_allclose(M[2][big], (M[0] * s2 * c2)[big], rtol=2e-5, atol=1e-12 * M[0].max())
+    assert np.all(M[3] == 0.0)
+
+
+# ---------------------------------------------------------------------------------------------------
+# reduced C3, C4, C5 (same structure, several tiles and a ragged tail), full maps
+# ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name", ["C3", "C4", "C5"])
+@pytest.mark.parametrize("variant", [0, 1])
+def test_small_config_maps(nms, ctx, oracle_mod, name, variant):
+    wl = ni.make_config(name, small=True)
+    kinds = list(ni.ALL_KINDS)
+    nms.nms_set_option(ctx, "variant", variant)
+    qy, qz, th = oracle_mod.grid_points(wl.grid)
+    rots = wl.rotations if wl.rotations is not None else [wl.R]
+    _upload(nms, ctx, wl)
+    for R in rots:
+        nms.nms_set_rotation(ctx, R)
+        A_gpu, M_gpu = _run_full(nms, ctx, wl, kinds)
+        A, wsum, M = _oracle_maps(oracle_mod, wl, qy, qz, th, kinds, R=R)
+        assert_amplitudes(A_gpu, A, wsum, name)
+        assert_cross_sections(M_gpu, M, kinds, name)
+
+
+def test_form_factor_split_small(nms, ctx, oracle_mod):
+    """Eq. 49-50: total = B(sum A_p), form = sum B(A_p); with and without separate object centres."""
+    import torch
+    for sep in (False, True):
+        wl = ni.config_c3(K=7, n_q=21, n_theta=40, separate_centres=sep)
+        kinds = list(ni.ALL_KINDS)
+        _upload(nms, ctx, wl)
+        qy, qz, th = oracle_mod.grid_points(wl.grid)
+        tot_ref, form_ref = oracle_mod.form_factor_split(wl.pos, wl.N, wl.m, wl.offsets, kinds, qy, qz, th, R=wl.R,
+                                                         centres=wl.centres, P=wl.P)
+        for chunks in (0, 1, 3):
+            nms.nms_set_option(ctx, "chunks", chunks)
+            tot = torch.empty((len(kinds), wl.grid.n_q), dtype=torch.float32, device="cuda")
+            form = torch.empty_like(tot)
+            nms.nms_form_factor_split(ctx, wl.grid, kinds, tot, form)
+            nms.nms_synchronize(ctx)
+            assert_cross_sections(tot.cpu().numpy(), tot_ref, kinds, "split total")
+            assert_cross_sections(form.cpu().numpy(), form_ref, kinds, "split form")
+        # the ordinary path gives the same total
+        maps = torch.empty_like(tot)
+        nms.nms_compute(ctx, wl.grid, kinds, maps)
+        nms.nms_synchronize(ctx)
+        assert_cross_sections(maps.cpu().numpy(), tot_ref, kinds, "ordinary total")
+
+
+def test_form_factor_split_uneven_objects(nms, ctx, oracle_mod):
+    """Objects of very different sizes (1 cell .. > 1 tile), one of them empty."""
+    import torch
+    rng = np.random.Generator(np.random.Philox(77))
+    sizes = [1, 0, 1500, 7, 1024, 2049, 33]
+    W = sum(sizes)
+    offsets = np.concatenate([[0], np.cumsum(sizes)]).astype(np.int64)
+    pos = rng.uniform(-30, 30, size=(W, 3)).astype(np.float32)
+    N = rng.uniform(0.5, 1.5, size=W).astype(np.float32)
+    m = rng.normal(size=(W, 3)).astype(np.float32)
+    cen = rng.uniform(-100, 100, size=(len(sizes), 3)).astype(np.float32)
+    R = ni.rotation_alpha_beta(20.0, 50.0)
+    grid = ni.polar_grid(0.02 * 1.3 ** np.arange(13), 24)
+    kinds = list(ni.ALL_KINDS)
+    nms.nms_set_sample(ctx, _t(pos), _t(N), _t(m), R)
+    nms.nms_set_particles(ctx, offsets, _t(cen))
+    qy, qz, th = oracle_mod.grid_points(grid)
+    tot_ref, form_ref = oracle_mod.form_factor_split(pos, N, m, offsets, kinds, qy, qz, th, R=R, centres=cen)
+    tot = torch.empty((len(kinds), grid.n_q), dtype=torch.float32, device="cuda")
+    form = torch.empty_like(tot)
+    nms.nms_form_factor_split(ctx, grid, kinds, tot, form)
+    nms.nms_synchronize(ctx)
+    assert_cross_sections(tot.cpu().numpy(), tot_ref, kinds, "uneven total")
+    assert_cross_sections(form.cpu().numpy(), form_ref, kinds, "uneven form")
+
+
+# ---------------------------------------------------------------------------------------------------
+# azimuthal average and correlation: pass-isolated (oracle pass on the GPU's own maps) and end to end
+# ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name", ["C1", "C2"])
+def test_azimuthal_and_correlation(nms, ctx, oracle_mod, name):
+    import torch
+    wl = ni.make_config(name)
+    kinds = wl.kinds
+    _upload(nms, ctx, wl)
+    nq = wl.grid.n_q
+    maps = torch.empty((len(kinds), nq), dtype=torch.float32, device="cuda")
+    nms.nms_compute(ctx, wl.grid, kinds, maps)
+    nb = wl.n_bins
+    I = torch.empty((len(kinds), nb), dtype=torch.float32, device="cuda")
+    qb = torch.empty(nb, dtype=torch.float32, device="cuda")
+    cnt = torch.empty(nb, dtype=torch.int32, device="cuda")
+    nms.nms_azimuthal_average(ctx, maps, len(kinds), nb, wl.q_lo, wl.q_hi, I, qb, cnt)
+    nms.nms_synchronize(ctx)
+    maps_h, I_h, qb_h, cnt_h = maps.cpu().numpy(), I.cpu().numpy(), qb.cpu().numpy(), cnt.cpu().numpy()
+    qy, qz, th = oracle_mod.grid_points(wl.grid)
+    if wl.grid.type == 0:
+        I_iso = oracle_mod.azimuthal_polar(maps_h, wl.grid.n0, wl.grid.n1)
+        cnt_ref = np.full(nb, wl.grid.n1, dtype=np.int32)
+        q_ref = wl.grid.u0.astype(np.float64)
+    else:
+        I_iso, cnt_ref = oracle_mod.azimuthal_hist(maps_h, qy, qz, nb, wl.q_lo, wl.q_hi)
+        q_ref = oracle_mod.hist_bin_centres(nb, wl.q_lo, wl.q_hi)
+    assert np.array_equal(cnt_h, cnt_ref)                       # integer work: bit exact
+    np.testing.assert_allclose(qb_h, q_ref, rtol=1e-6)
+    scale = np.abs(I_iso).max(axis=1, keepdims=True)
+    assert np.all(np.abs(I_h - I_iso) <= 2e-7 * scale + 1e-6 * np.abs(I_iso))   # pass-isolated: fp32 output rounding only
+    # end to end against the oracle's own maps
+    A, wsum, M = _oracle_maps(oracle_mod, wl, qy, qz, th, kinds)
+    I_ref = oracle_mod.azimuthal_polar(M, wl.grid.n0, wl.grid.n1) if wl.grid.type == 0 else oracle_mod.azimuthal_hist(M, qy, qz, nb, wl.q_lo, wl.q_hi)[0]
+    assert_cross_sections(I_h, I_ref, kinds, name + " I(q)")
+    # correlation function
+    r = wl.r if wl.r is not None else np.linspace(0.0, 25.0, 64).astype(np.float32)
+    r_d = _t(r)
+    c = torch.empty((len(kinds), len(r)), dtype=torch.float32, device="cuda")
+    p = torch.empty_like(c)
+    nms.nms_correlation(ctx, I, qb, cnt, len(kinds), nb, r_d, c, p)
+    nms.nms_synchronize(ctx)
+    c_iso, p_iso = oracle_mod.correlation(I_h, qb_h, r, count=cnt_h)
+    for got, want in ((c.cpu().numpy(), c_iso), (p.cpu().numpy(), p_iso)):
+        sc = np.abs(want).max(axis=1, keepdims=True)
+        assert np.all(np.abs(got - want) <= 3e-7 * sc + 1e-6 * np.abs(want))
+    c_ref, p_ref = oracle_mod.correlation(I_ref, q_ref, r, count=cnt_ref)
+    assert_cross_sections(c.cpu().numpy(), c_ref, kinds, name + " c(r)")
+    assert_cross_sections(p.cpu().numpy(), p_ref, kinds, name + " p(r)")
+
+
+def test_histogram_on_polar_grid_and_empty_bins(nms, ctx, oracle_mod):
+    import torch
+    wl = ni.make_config("C1")
+    _upload(nms, ctx, wl)
+    kinds = [KI["NUC"], KI["NM"]]
+    maps = torch.empty((2, wl.grid.n_q), dtype=torch.float32, device="cuda")
+    nms.nms_compute(ctx, wl.grid, kinds, maps)
+    nb = 200                                                       # finer than the 64 rings: many empty bins
+    I = torch.empty((2, nb), dtype=torch.float32, device="cuda")
+    cnt = torch.empty(nb, dtype=torch.int32, device="cuda")
+    nms.nms_azimuthal_average(ctx, maps, 2, nb, 0.5, 2.0, I, None, cnt)
+    nms.nms_synchronize(ctx)
+    qy, qz, _ = oracle_mod.grid_points(wl.grid)
+    I_ref, cnt_ref = oracle_mod.azimuthal_hist(maps.cpu().numpy(), qy, qz, nb, 0.5, 2.0)
+    assert np.array_equal(cnt.cpu().numpy(), cnt_ref)
+    assert (cnt_ref == 0).sum() > 50
+    np.testing.assert_allclose(I.cpu().numpy(), I_ref, rtol=2e-6, atol=0)
+
+
+# ---------------------------------------------------------------------------------------------------
+# edge cases
+# ---------------------------------------------------------------------------------------------------
+def test_list_grid_with_q_zero_gives_weight_sums(nms, ctx):
+    """F(0) = sum w (north_star) through the GPU path; theta(0,0) = 0 (reading 5)."""
+    import torch
+    rng = np.random.Generator(np.random.Philox(5))
+    W = 3001
+    pos = rng.normal(scale=20, size=(W, 3)).astype(np.float32)
+    N = rng.normal(size=W).astype(np.float32)
+    m = rng.normal(size=(W, 3)).astype(np.float32)
+    R = ni.rotation_alpha_beta(10.0, 20.0)
+    nms.nms_set_sample(ctx, _t(pos), _t(N), _t(m), R)
+    grid = ni.list_grid(np.zeros(3), np.zeros(3))
+    amp = torch.empty((8, 3), dtype=torch.float32, device="cuda")
+    nms.nms_amplitudes(ctx, grid, amp)
+    nms.nms_synchronize(ctx)
+    a = amp.cpu().numpy().astype(np.float64)
+    ms = R @ m.astype(np.float64).sum(axis=0)
+    want = np.array([N.astype(np.float64).sum(), 0, ms[0], 0, ms[1], 0, ms[2], 0])
+    wsum = nms.nms_get_weight_sums(ctx)
+    for j in range(3):
+        assert np.all(np.abs(a[:, j] - want) <= 1e-6 * np.repeat(wsum, 2) + 1e-30)
+
+
+@pytest.mark.parametrize("W", [1, 2, 7, 8, 9, 1023, 1024, 1025, 2055])
+def test_ragged_cell_counts(nms, ctx, oracle_mod, W):
+    import torch
+    rng = np.random.Generator(np.random.Philox(100 + W))
+    pos = rng.uniform(-15, 15, size=(W, 3)).astype(np.float32)
+    N = rng.uniform(-1, 1, size=W).astype(np.float32)
+    m = rng.normal(size=(W, 3)).astype(np.float32)
+    nms.nms_set_sample(ctx, _t(pos), _t(N), _t(m), None)
+    grid = ni.polar_grid(np.linspace(0.05, 2.0, 19), 37)              # 19 rings: ragged against QT = 4, 8, 16
+    qy, qz, th = oracle_mod.grid_points(grid)
+    A, wsum = oracle_mod.amplitudes(pos, N, m, None, qy, qz, return_wsum=True)
+    for qt in (4, 8, 16):
+        nms.nms_set_option(ctx, "qt", qt)
+        amp = torch.empty((8, grid.n_q), dtype=torch.float32, device="cuda")
+        nms.nms_amplitudes(ctx, grid, amp)
+        nms.nms_synchronize(ctx)
+        assert_amplitudes(amp.cpu().numpy(), A, wsum, f"W={W} qt={qt}")
+
+
+def test_absent_channels(nms, ctx, oracle_mod):
+    """N == NULL / m == NULL switch a channel off (L242): its amplitudes are exactly zero."""
+    import torch
+    wl = ni.make_config("C5", small=True)
+    qy, qz, th = oracle_mod.grid_points(wl.grid)
+    for N, m in ((wl.N, None), (None, wl.m)):
+        nms.nms_set_sample(ctx, _t(wl.pos), _t(N), _t(m), None)
+        amp = torch.empty((8, wl.grid.n_q), dtype=torch.float32, device="cuda")
+        nms.nms_amplitudes(ctx, wl.grid, amp)
+        nms.nms_synchronize(ctx)
+        A, wsum = oracle_mod.amplitudes(wl.pos, N, m, None, qy, qz, return_wsum=True)
+        assert_amplitudes(amp.cpu().numpy(), A, wsum, "absent channel")
+
+
+def test_general_polarization_and_scales(nms, ctx, oracle_mod):
+    import torch
+    wl = ni.make_config("C2")
+    wl.P = np.array([0.3, -0.5, 0.8])
+    _upload(nms, ctx, wl)
+    nms.nms_set_scales(ctx, 2.5e-3, 0.7, 1.0 / 37.0)
+    kinds = list(ni.ALL_KINDS)
+    maps = torch.empty((len(kinds), wl.grid.n_q), dtype=torch.float32, device="cuda")
+    nms.nms_compute(ctx, wl.grid, kinds, maps)
+    nms.nms_synchronize(ctx)
+    qy, qz, th = oracle_mod.grid_points(wl.grid)
+    A = oracle_mod.amplitudes(wl.pos, wl.N, wl.m, wl.R, qy, qz)
+    M = oracle_mod.response(A, th, kinds, P=wl.P, sN=2.5e-3, sM=0.7, invV=1.0 / 37.0)
+    assert_cross_sections(maps.cpu().numpy(), M, kinds, "general P")
+
+
+def test_error_codes(nms, ctx):
+    import torch
+    wl = ni.make_config("C1")
+    pos, N, m = _t(wl.pos), _t(wl.N), _t(wl.m)
+    out = torch.empty((1, wl.grid.n_q), dtype=torch.float32, device="cuda")
+
+    def status(fn, *a):
+        with pytest.raises(nms.NmsError) as e:
+            fn(*a)
+        return e.value.status
+
+    assert status(nms.nms_compute, ctx, wl.grid, [0], out) == nms.NMS_E_STATE            # no sample yet
+    assert status(nms.nms_set_sample, ctx, pos, None, None, None) == nms.NMS_E_ARG        # no weights
+    assert status(nms.nms_set_sample, ctx, pos, N, m, np.eye(3) * 1.01) == nms.NMS_E_ARG  # R not orthonormal
+    nms.nms_set_sample(ctx, pos, N, m, None)
+    assert status(nms.nms_response, ctx, [0], out) == nms.NMS_E_STATE                     # before nms_amplitudes
+    assert status(nms.nms_compute, ctx, wl.grid, [99], out) == nms.NMS_E_ARG              # unknown kind
+    assert status(nms.nms_form_factor_split, ctx, wl.grid, [0], out, out) == nms.NMS_E_STATE   # no particles
+    assert status(nms.nms_set_particles, ctx, np.array([0, 5, 3, wl.W]), None) == nms.NMS_E_ARG
+    assert status(nms.nms_set_particles, ctx, np.array([0, 5, wl.W - 1]), None) == nms.NMS_E_ARG
+    assert status(nms.nms_set_polarization, ctx, [0, 0, 0]) == nms.NMS_E_ARG
+    assert status(nms.nms_set_option, ctx, "nonsense", 1) == nms.NMS_E_ARG
+    bad = ni.polar_grid(0.01 * 1.5 ** np.arange(8), 8)
+    nms.nms_set_option(ctx, "variant", 2)
+    assert status(nms.nms_compute, ctx, bad, [0], out[:, :64].contiguous()) == nms.NMS_E_UNSUPPORTED
+    nms.nms_set_option(ctx, "variant", 0)
+    nms.nms_compute(ctx, wl.grid, [0], out)                                             # context still usable
+    nms.nms_synchronize(ctx)
+    assert "" == nms.nms_last_error(ctx)
+
+
+def test_run_host_matches_device_path(nms, ctx):
+    import torch
+    wl = ni.make_config("C2")
+    kinds = wl.kinds
+    nq, nb, nr = wl.grid.n_q, wl.n_bins, len(wl.r)
+    out_maps = np.empty((len(kinds), nq), dtype=np.float32)
+    out_I = np.empty((len(kinds), nb), dtype=np.float32)
+    out_c = np.empty((len(kinds), nr), dtype=np.float32)
+    out_p = np.empty_like(out_c)
+    nms.nms_run_host(ctx, wl.pos, wl.N, wl.m, wl.R, wl.grid, kinds, out_maps, nb, wl.q_lo, wl.q_hi, out_I, wl.r, out_c, out_p)
+    _upload(nms, ctx, wl)
+    maps = torch.empty((len(kinds), nq), dtype=torch.float32, device="cuda")
+    nms.nms_compute(ctx, wl.grid, kinds, maps)
+    nms.nms_synchronize(ctx)
+    assert np.array_equal(maps.cpu().numpy(), out_maps)
+    assert np.isfinite(out_I).all() and np.isfinite(out_c).all() and np.isfinite(out_p).all()
