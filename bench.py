@@ -1,0 +1,468 @@
+#!/usr/bin/env python3
+"""bench.py -- throughput of the direct-summation SANS hot path on B200 (contract: see DESIGN.md section 8).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C5] [--impl reference]
+
+One "step" is one pass of the whole hot path over one synthetic workload whose raw arrays are already
+resident in HBM: a-1 prep (rotate + order + pack), a-2 amplitude sums, a-3 reduce + response epilogue,
+and, where the config asks for them, a-4 azimuthal average, a-5 correlation function, a-6 form-factor
+split.  The metric is BASELINE.json's: Gpair/s = W * n_q * n_rotations * n_gpus / t, pairs actually
+evaluated (no symmetry or merging tricks).  Rank 0 prints ONE JSON line.
+
+ * value        device-resident inputs, CUDA events on the launching stream, max over ranks
+ * e2e          same step through the C ABI with HOST buffers (pinned), H2D and D2H copies inside the
+                timed region
+ * roofline     the amplitude kernel: 12 FP32 lane-instructions per pair over its
+                CUDA-event time inside the timed region, against N_SM * 128 lanes * sm_max_mhz
+ * cpu_baseline the fp64 oracle as it stands, timed on this box's host cores on a bounded sample
+ * --impl reference   the oracle alone (this tier's reference arm), same metric and config
+
+N > 1 (torchrun): the path runs on one GPU (north_star); every rank runs an independent replica of the
+workload on its own GPU ("replicas only"), no data-path collective; value = total
+pairs of all ranks / max-over-ranks time; scaling = weak.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import nms_inputs as ni  # noqa: E402  (seeded input generators only; no arithmetic of the method)
+
+FP32_LANE_INSTR_PER_PAIR = 12      # 8 accumulate FFMA + 4 for the phasor
+LANES_PER_SM = 128
+
+
+def _env_int(name, default):
+    try:
+        return int(os.environ.get(name, default))
+    except ValueError:
+        return default
+
+
+def _peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return json.load(f), "MEASURED_PEAKS.json"
+    # fallback of /opt/skills/guides/B200_PROFILING.md: nominal B200 numbers
+    return {"hbm_gbs": 7700.0, "sm_max_mhz": 1965.0}, "B200_PROFILING.md fallback (nominal)"
+
+
+# ---------------------------------------------------------------------------------------------------
+# clocks: sample NVML during the timed region
+# ---------------------------------------------------------------------------------------------------
+class ClockSampler:
+    REASONS = {0x1: "gpu_idle", 0x2: "applications_clocks_setting", 0x4: "sw_power_cap", 0x8: "hw_slowdown",
+               0x10: "sync_boost", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+               0x80: "hw_power_brake_slowdown", 0x100: "display_clock_setting"}
+
+    def __init__(self, index: int, period: float = 0.05):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thr = None
+        self.period = period
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self.nv = None
+
+    def _run(self):
+        while not self._stop.is_set():
+            try:
+                self.samples.append(float(self.nv.nvmlDeviceGetClockInfo(self.h, self.nv.NVML_CLOCK_SM)))
+                bits = int(self.nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                for b, name in self.REASONS.items():
+                    if bits & b and name != "gpu_idle":
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            self._stop.wait(self.period)
+
+    def start(self):
+        if self.nv is not None:
+            self._stop.clear()
+            self._thr = threading.Thread(target=self._run, daemon=True)
+            self._thr.start()
+
+    def stop(self):
+        if self._thr is not None:
+            self._stop.set()
+            self._thr.join()
+            self._thr = None
+
+    def summary(self):
+        med = float(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+# ---------------------------------------------------------------------------------------------------
+# the CUDA arm
+# ---------------------------------------------------------------------------------------------------
+class Runner:
+    """Owns one context, the device-resident raw arrays of one workload and its output buffers."""
+
+    def __init__(self, nms, wl, device: int):
+        import torch
+        self.nms, self.wl, self.torch = nms, wl, torch
+        self.dev = torch.device("cuda", device)
+        self.ctx = nms.Context(device)
+        self.h = self.ctx.h
+        pin = lambda a: None if a is None else torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+        self.h_pos, self.h_N, self.h_m = pin(wl.pos), pin(wl.N), pin(wl.m)
+        self.h_cen = pin(wl.centres)
+        up = lambda t: None if t is None else t.to(self.dev, non_blocking=True)
+        self.d_pos, self.d_N, self.d_m, self.d_cen = up(self.h_pos), up(self.h_N), up(self.h_m), up(self.h_cen)
+        nk, nq = len(wl.kinds), wl.grid.n_q
+        f32 = dict(dtype=torch.float32, device=self.dev)
+        self.maps = torch.empty((nk, nq), **f32)
+        self.form = torch.empty((nk, nq), **f32) if wl.split else None
+        self.h_maps = torch.empty((nk, nq), dtype=torch.float32).pin_memory()
+        self.h_form = torch.empty((nk, nq), dtype=torch.float32).pin_memory() if wl.split else None
+        self.nb = wl.n_bins
+        if self.nb:
+            self.I = torch.empty((nk, self.nb), **f32)
+            self.qb = torch.empty(self.nb, **f32)
+            self.cnt = torch.empty(self.nb, dtype=torch.int32, device=self.dev)
+            self.h_I = torch.empty((nk, self.nb), dtype=torch.float32).pin_memory()
+        self.nr = 0 if wl.r is None else len(wl.r)
+        if self.nr:
+            self.h_r = pin(wl.r)
+            self.d_r = up(self.h_r)
+            self.c = torch.empty((nk, self.nr), **f32)
+            self.p = torch.empty((nk, self.nr), **f32)
+            self.h_c = torch.empty((nk, self.nr), dtype=torch.float32).pin_memory()
+            self.h_p = torch.empty((nk, self.nr), dtype=torch.float32).pin_memory()
+        self.rots = wl.rotations if wl.rotations is not None else [wl.R]
+        torch.cuda.synchronize(self.dev)
+
+    # -- one pass of the hot path, raw arrays resident in HBM -------------------------------------------
+    def _post(self):
+        nms, wl, h = self.nms, self.wl, self.h
+        if self.nb:
+            nms.nms_azimuthal_average(h, self.maps, len(wl.kinds), self.nb, wl.q_lo, wl.q_hi, self.I, self.qb, self.cnt)
+            if self.nr:
+                nms.nms_correlation(h, self.I, self.qb, self.cnt, len(wl.kinds), self.nb, self.d_r, self.c, self.p)
+
+    def step_device(self, d2h: bool = False):
+        nms, wl, h = self.nms, self.wl, self.h
+        nms.nms_set_sample(h, self.d_pos, self.d_N, self.d_m, self.rots[0])          # a-1
+        if wl.offsets is not None:
+            nms.nms_set_particles(h, wl.offsets, self.d_cen)
+        nms.nms_set_polarization(h, wl.P)
+        for i, R in enumerate(self.rots):
+            if i > 0:
+                nms.nms_set_rotation(h, R)                                            # a-1 again (rocking scan)
+            if wl.split:
+                nms.nms_form_factor_split(h, wl.grid, wl.kinds, self.maps, self.form)  # a-6 (+ a-2, a-3)
+            else:
+                nms.nms_compute(h, wl.grid, wl.kinds, self.maps)                       # a-2 + a-3
+            self._post()                                                              # a-4, a-5
+            if d2h:
+                self.h_maps.copy_(self.maps, non_blocking=True)
+                if wl.split:
+                    self.h_form.copy_(self.form, non_blocking=True)
+                if self.nb:
+                    self.h_I.copy_(self.I, non_blocking=True)
+                if self.nr:
+                    self.h_c.copy_(self.c, non_blocking=True)
+                    self.h_p.copy_(self.p, non_blocking=True)
+
+    # -- the same step from HOST buffers: H2D of the raw arrays and D2H of every result inside ------------
+    def step_host(self):
+        nms, wl, h, torch = self.nms, self.wl, self.h, self.torch
+        if wl.split or len(self.rots) > 1:
+            # nms_run_host covers one rotation without object structure; here the binding-level calls are
+            # used with explicit pinned copies (nms_set_sample accepts host pointers through UVA as well)
+            self.d_pos.copy_(self.h_pos, non_blocking=True)
+            if self.d_N is not None:
+                self.d_N.copy_(self.h_N, non_blocking=True)
+            if self.d_m is not None:
+                self.d_m.copy_(self.h_m, non_blocking=True)
+            if self.d_cen is not None:
+                self.d_cen.copy_(self.h_cen, non_blocking=True)
+            self.step_device(d2h=True)
+            torch.cuda.current_stream(self.dev).synchronize()
+        else:
+            nms.nms_run_host(h, self.h_pos, self.h_N, self.h_m, wl.R, wl.grid, wl.kinds, self.h_maps, self.nb, wl.q_lo,
+                             wl.q_hi, self.h_I if self.nb else None, self.h_r if self.nr else None,
+                             self.h_c if self.nr else None, self.h_p if self.nr else None)
+
+    def bytes_per_step(self):
+        wl = self.wl
+        h2d = sum(t.numel() * t.element_size() for t in (self.h_pos, self.h_N, self.h_m, self.h_cen) if t is not None)
+        per_rot = self.h_maps.numel() * 4 + (self.h_form.numel() * 4 if wl.split else 0)
+        if self.nb:
+            per_rot += self.h_I.numel() * 4
+        if self.nr:
+            h2d += self.h_r.numel() * 4
+            per_rot += 2 * self.h_c.numel() * 4
+        return int(h2d), int(per_rot * len(self.rots))
+
+    def close(self):
+        self.ctx.close()
+
+
+def _timed(torch, dev, fn, steps, dist=None):
+    """Time exactly `steps` calls of fn between barrier + synchronize on both sides; ms, max over ranks."""
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize(dev)
+    beg, end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    beg.record()
+    for _ in range(steps):
+        fn()
+    end.record()
+    torch.cuda.synchronize(dev)
+    ms = beg.elapsed_time(end)
+    if dist is not None:
+        dist.barrier()
+    return max_over_ranks(ms, dist, torch, dev)
+
+
+def max_over_ranks(value: float, dist=None, torch=None, dev=None) -> float:
+    """MAX-reduce a scalar over the process group (identity without one).  Works on gloo (CPU) and nccl."""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return float(value)
+    import torch as _t
+    t = _t.tensor([float(value)], dtype=_t.float64, device=dev if dist.get_backend() == "nccl" else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_rate(pairs_per_rank: int, world: int, ms_max: float) -> float:
+    """Whole-job Gpair/s: every rank evaluated pairs_per_rank pairs in (max over ranks) ms_max."""
+    return pairs_per_rank * world / (ms_max * 1e-3) / 1e9
+
+
+# ---------------------------------------------------------------------------------------------------
+# the oracle arm (cpu_baseline leg and --impl reference): the only places bench.py executes oracle/
+# ---------------------------------------------------------------------------------------------------
+def oracle_step(oracle, wl, qy, qz, th, idx):
+    """One bounded sample of the workload through the fp64 oracle as it stands: all cells x the detector
+    points idx (first rotation only), responses, and the 1-D passes when the sample is the full detector."""
+    full = len(idx) == wl.grid.n_q
+    R = wl.rotations[0] if wl.rotations is not None else wl.R
+    if wl.split:
+        tot, form = oracle.form_factor_split(wl.pos, wl.N, wl.m, wl.offsets, wl.kinds, qy[idx], qz[idx], th[idx], R=R,
+                                             centres=wl.centres, P=wl.P)
+        return tot
+    A = oracle.amplitudes(wl.pos, wl.N, wl.m, R, qy[idx], qz[idx], offsets=wl.offsets, centres=wl.centres)
+    M = oracle.response(A, th[idx], wl.kinds, P=wl.P)
+    if full and wl.n_bins:
+        if wl.grid.type == 0 and not (wl.q_hi > wl.q_lo):
+            I = oracle.azimuthal_polar(M, wl.grid.n0, wl.grid.n1)
+            qb, cnt = wl.grid.u0.astype(np.float64), None
+        else:
+            I, cnt = oracle.azimuthal_hist(M, qy, qz, wl.n_bins, wl.q_lo, wl.q_hi)
+            qb = oracle.hist_bin_centres(wl.n_bins, wl.q_lo, wl.q_hi)
+        if wl.r is not None:
+            oracle.correlation(I, qb, wl.r, count=cnt)
+    return M
+
+
+def oracle_sample(wl, n_sample):
+    n = min(n_sample, wl.grid.n_q)
+    if n == wl.grid.n_q:
+        return np.arange(n, dtype=np.int64)
+    return ni.q_subset(wl.grid.n_q, n, 9000 + int(wl.name[1]))
+
+
+def time_oracle(wl, target_s=12.0, steps=1, warmup=0):
+    """Gpair/s of the oracle on a sample sized for about target_s seconds per step (probe first, then scale)."""
+    import oracle
+    oracle.build()
+    qy, qz, th = oracle.grid_points(wl.grid)
+    n = 8
+    while True:                                        # probe with growing samples until the timing is meaningful
+        probe = oracle_sample(wl, n)
+        t0 = time.perf_counter()
+        oracle_step(oracle, wl, qy, qz, th, probe)
+        el = time.perf_counter() - t0
+        if el >= 0.5 or len(probe) == wl.grid.n_q:
+            break
+        n *= 8
+    rate = wl.W * len(probe) / max(el, 1e-9)
+    n = int(max(8, min(wl.grid.n_q, rate * target_s / wl.W)))
+    idx = oracle_sample(wl, n)
+    for _ in range(warmup):
+        oracle_step(oracle, wl, qy, qz, th, idx)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        oracle_step(oracle, wl, qy, qz, th, idx)
+    dt = (time.perf_counter() - t0) / steps
+    pairs = wl.W * len(idx)
+    return {"value": pairs / dt / 1e9, "unit": "Gpair/s", "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": f"all {wl.W} cells x {len(idx)} of {wl.grid.n_q} detector points (seeded subset, first rotation), "
+                      f"fp64, {dt:.2f} s per step"}, dt * 1e3
+
+
+def metric_name():
+    with open(os.path.join(ROOT, "BASELINE.json")) as f:
+        return json.load(f)["metric"]
+
+
+def workload_config(wl, extra=None):
+    g = wl.grid
+    cfg = {"workload": f"{wl.name}: {WORKLOAD_TEXT[wl.name]}", "cells": wl.W,
+           "detector": f"{['polar', 'cartesian', 'list'][g.type]} {g.n0}x{g.n1}", "n_q": g.n_q, "rotations": wl.n_rot,
+           "pairs_per_step": wl.pairs, "kinds": [ni.KINDS[k] for k in wl.kinds],
+           "cache": "inputs larger than L2" if wl.W * 28 > 126e6 else "inputs fit in L2; each step re-packs them"}
+    if extra:
+        cfg.update(extra)
+    return cfg
+
+
+WORKLOAD_TEXT = {
+    "C1": "uniformly magnetized sphere, 1 nm cells, R = 10 nm",
+    "C2": "vortex disc, 2 nm cells, rotated ZYZ (30,45,0) deg, all responses, I(q), c(r), p(r)",
+    "C3": "ensemble of 1000 spheres (R = 5 nm, 0.5 nm cells), total and form-factor outputs",
+    "C4": "skyrmion-lattice film 512x512x8, rocking scan of 36 rotations about z",
+    "C5": "micromagnetic block 256^3 with 5 % pores, all responses, I(q), c(r), p(r)",
+}
+
+
+def run_reference(args, rank):
+    if rank != 0:
+        return
+    wl = ni.make_config(args.workload)
+    cb, ms = time_oracle(wl, target_s=args.oracle_seconds, steps=max(args.steps, 1), warmup=min(args.warmup, 1))
+    line = {"impl": "reference", "metric": metric_name(), "value": cb["value"], "unit": "Gpair/s", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": min(args.warmup, 1), "ms_per_step": ms, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": workload_config(wl), "cpu_baseline": cb,
+            "e2e": {"value": cb["value"], "unit": "Gpair/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def run_cuda(args, rank, local_rank, world):
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product has no CPU fallback (use --impl reference for the oracle)")
+    import paper_2601_18444_b200 as nms       # raises if libnms.so is missing and cannot be built
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        torch.cuda.set_device(local_rank)
+        dist.init_process_group(backend="nccl", device_id=torch.device("cuda", local_rank))
+    dev = torch.device("cuda", local_rank)
+    torch.cuda.set_device(dev)
+
+    wl = ni.make_config(args.workload)
+    run = Runner(nms, wl, local_rank)
+    h = run.h
+    sampler = ClockSampler(local_rank)
+
+    # ---- device-resident arm -------------------------------------------------------------------------
+    for _ in range(args.warmup):
+        run.step_device()
+    nms.nms_synchronize(h)
+    launches0 = nms.nms_get_info(h, "launches")
+    nms.nms_set_option(h, "timing", 1)                 # event pair around every kernel; resets the record
+    sampler.start()
+    ms_total = _timed(torch, dev, run.step_device, args.steps, dist)
+    sampler.stop()
+    launches = nms.nms_get_info(h, "launches") - launches0
+    kt = {name: nms.nms_kernel_time_total(h, idx) for name, idx in
+          (("prep", nms.NMS_T_PREP), ("amplitude", nms.NMS_T_AMPLITUDE), ("epilogue", nms.NMS_T_EPILOGUE),
+           ("azimuthal", nms.NMS_T_AZIMUTHAL), ("correlation", nms.NMS_T_CORRELATION))}
+    nms.nms_set_option(h, "timing", 0)
+    ms_step = ms_total / args.steps
+    value = aggregate_rate(wl.pairs, world, ms_step)
+
+    # ---- roofline of the dominant kernel (amplitude sums) --------------------------------------------
+    peaks, peak_src = _peaks()
+    sm_count = nms.nms_get_info(h, "sm_count")
+    amp_ms, amp_n = kt["amplitude"]
+    amp_ms_per_launch = amp_ms / max(amp_n, 1)
+    pairs_per_launch = wl.W * wl.grid.n_q
+    achieved = pairs_per_launch * FP32_LANE_INSTR_PER_PAIR / (amp_ms_per_launch * 1e-3) / 1e12
+    peak = sm_count * LANES_PER_SM * peaks["sm_max_mhz"] * 1e6 / 1e12
+    clocks = sampler.summary()
+    roofline = {"bound": "alu", "kernel": "k_amp (a-2 amplitude sums)", "achieved": achieved, "peak": peak,
+                "unit": "T FP32 lane-instr/s (12 per pair)", "frac": achieved / peak, "traffic": None,
+                "peak_source": f"{sm_count} SMs x 128 FP32 lanes x sm_max_mhz {peaks['sm_max_mhz']:.0f} ({peak_src})",
+                "gpair_s_kernel": pairs_per_launch / (amp_ms_per_launch * 1e-3) / 1e9,
+                "ms_per_launch": amp_ms_per_launch, "launches_timed": amp_n,
+                "share_of_step": amp_ms / ms_total,
+                "frac_at_sampled_clock": (achieved / (sm_count * LANES_PER_SM * clocks["sm_mhz"] * 1e6 / 1e12))
+                if clocks.get("sm_mhz") else None,
+                "variant": nms.nms_get_info(h, "variant_used"), "qt": nms.nms_get_info(h, "qt"),
+                "cell_chunks": nms.nms_get_info(h, "n_chunks"), "blocks_per_sm": nms.nms_get_info(h, "blocks_per_sm")}
+    passes = {}
+    hbm = peaks.get("hbm_gbs", 0.0)
+    nk, nq = len(wl.kinds), wl.grid.n_q
+    alg_bytes = {"prep": wl.W * 52.0,                                       # 28 B in, 24 B out per cell (a-1)
+                 "azimuthal": nk * nq * 4.0 + nk * max(wl.n_bins, 1) * 4.0,  # maps in, I(q) out (a-4)
+                 "correlation": nk * max(wl.n_bins, 1) * 4.0 + 2.0 * nk * max(run.nr, 1) * 4.0}   # a-5
+    for name in ("prep", "epilogue", "azimuthal", "correlation"):
+        t, n = kt[name]
+        if n:
+            passes[name] = {"ms_per_launch": t / n, "launches": n}
+            if name in alg_bytes:
+                gbs = alg_bytes[name] / (t / n * 1e-3) / 1e9
+                passes[name].update({"achieved_gbs": gbs, "frac_of_hbm_peak": gbs / hbm if hbm else None})
+
+    # ---- end-to-end arm: host buffers, copies inside the timed region --------------------------------
+    for _ in range(min(args.warmup, 2)):
+        run.step_host()
+    e2e_steps = max(1, min(args.steps, 3))
+    ms_e2e = _timed(torch, dev, run.step_host, e2e_steps, dist) / e2e_steps
+    h2d, d2h = run.bytes_per_step()
+    e2e = {"value": aggregate_rate(wl.pairs, world, ms_e2e), "unit": "Gpair/s", "ms_per_step": ms_e2e,
+           "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": e2e_steps}
+    run.close()
+
+    cpu_baseline = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cpu_baseline, _ = time_oracle(wl, target_s=args.oracle_seconds)
+
+    if rank == 0:
+        line = {"metric": metric_name(), "value": value, "unit": "Gpair/s", "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": workload_config(wl, {"parallelism": "replicas only" if world > 1 else "single GPU"}),
+                "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "passes": passes,
+                "cpu_baseline": cpu_baseline}
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="C5", choices=["C1", "C2", "C3", "C4", "C5"])
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--oracle-seconds", type=float, default=12.0, help="CPU seconds per oracle step (bounded sample)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank, local_rank, world = _env_int("RANK", 0), _env_int("LOCAL_RANK", 0), _env_int("WORLD_SIZE", 1)
+    if world != args.gpus and world > 1:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}")
+    if args.gpus > 1 and world == 1:
+        raise SystemExit("bench.py: for --gpus N > 1 launch with python -m torch.distributed.run --nproc-per-node N")
+    if args.impl == "reference":
+        run_reference(args, rank)
+    else:
+        run_cuda(args, rank, local_rank, world)
+
+
+if __name__ == "__main__":
+    main()

@@ -196,7 +196,7 @@ NMS_API nms_status nms_get_weight_sums(nms_ctx* ctx, double* out);
 
 /* Integer options.  "variant": 0 auto, 1 force the direct (MUFU per pair) kernel, 2 force the
  * recurrence kernel (NMS_E_UNSUPPORTED at compute time if the detector lines are not equally spaced).
- * "timing": 1 records CUDA events around each kernel.  "chunks": 0 auto, else the number of cell
+ * "timing": 1 records a CUDA event pair around every kernel launch (and resets the record).  "chunks": 0 auto, else the number of cell
  * chunks.  "qt": 0 auto, else detector points per thread (4, 8 or 16).  Unknown keys: NMS_E_ARG. */
 NMS_API nms_status nms_set_option(nms_ctx* ctx, const char* key, int64_t value);
 /* Read back integers: "launches" (kernels launched by this context so far), "variant_used" (1 general
@@ -206,6 +206,10 @@ NMS_API nms_status nms_get_info(nms_ctx* ctx, const char* key, int64_t* value);
 /* Device time in ms of the most recent launch of the given kernel class ("timing" must be 1);
  * synchronises on that kernel's end event.  NMS_E_STATE if it has not run.                       */
 NMS_API nms_status nms_kernel_time_ms(nms_ctx* ctx, nms_timer which, float* ms);
+/* Sum of the device times [ms] and the number of launches of the given kernel class recorded since
+ * "timing" was last set (setting the option resets the record); synchronises on the recorded events.
+ * This is what bench.py divides the algorithmic work by for the roofline figure.                  */
+NMS_API nms_status nms_kernel_time_total(nms_ctx* ctx, nms_timer which, double* total_ms, int64_t* count);
 
 #ifdef __cplusplus
 }

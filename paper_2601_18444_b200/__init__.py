@@ -33,7 +33,7 @@ EXPORTS = [
     "nms_create", "nms_destroy", "nms_last_error", "nms_synchronize", "nms_set_sample", "nms_set_particles",
     "nms_set_rotation", "nms_set_polarization", "nms_set_scales", "nms_amplitudes", "nms_response", "nms_compute",
     "nms_azimuthal_average", "nms_correlation", "nms_form_factor_split", "nms_run_host", "nms_get_weight_sums",
-    "nms_set_option", "nms_get_info", "nms_kernel_time_ms",
+    "nms_set_option", "nms_get_info", "nms_kernel_time_ms", "nms_kernel_time_total",
 ]
 
 
@@ -233,6 +233,13 @@ def nms_kernel_time_ms(ctx, which: int) -> float:
     ms = C.c_float(0.0)
     _check(ctx, _lib.nms_kernel_time_ms(ctx, C.c_int(which), C.byref(ms)))
     return float(ms.value)
+
+
+def nms_kernel_time_total(ctx, which: int):
+    """(total_ms, launches) of a kernel class since "timing" was last set."""
+    tot, cnt = C.c_double(0.0), C.c_int64(0)
+    _check(ctx, _lib.nms_kernel_time_total(ctx, C.c_int(which), C.byref(tot), C.byref(cnt)))
+    return float(tot.value), int(cnt.value)
 
 
 class Context:

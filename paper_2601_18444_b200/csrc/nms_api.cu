@@ -46,15 +46,19 @@ void timer_begin(nms_ctx* c, int which)
 {
     if (!c->opt_timing) return;
     Timer& t = c->timers[which];
-    if (!t.beg) { cudaEventCreate(&t.beg); cudaEventCreate(&t.end); }
-    cudaEventRecord(t.beg, c->stream);
+    if (t.used == t.beg.size()) {
+        cudaEvent_t b = nullptr, e = nullptr;
+        cudaEventCreate(&b); cudaEventCreate(&e);
+        t.beg.push_back(b); t.end.push_back(e);
+    }
+    cudaEventRecord(t.beg[t.used], c->stream);
 }
 void timer_end(nms_ctx* c, int which)
 {
     if (!c->opt_timing) return;
     Timer& t = c->timers[which];
-    cudaEventRecord(t.end, c->stream);
-    t.ran = true;
+    cudaEventRecord(t.end[t.used], c->stream);
+    t.used += 1;
 }
 
 static void free_buf(DevBuf& b)
@@ -242,8 +246,8 @@ void nms_destroy(nms_ctx* c)
     for (DevBuf* b : bufs) free_buf(*b);
     for (DevBuf& b : c->host_stage) free_buf(b);
     for (Timer& t : c->timers) {
-        if (t.beg) cudaEventDestroy(t.beg);
-        if (t.end) cudaEventDestroy(t.end);
+        for (cudaEvent_t e : t.beg) cudaEventDestroy(e);
+        for (cudaEvent_t e : t.end) cudaEventDestroy(e);
     }
     delete c;
 }
@@ -447,7 +451,7 @@ nms_status nms_set_option(nms_ctx* c, const char* key, int64_t value)
     CHECK_CTX(c);
     if (!key) return fail(c, NMS_E_ARG, "key is NULL");
     if (!strcmp(key, "variant")) { if (value < 0 || value > 2) return fail(c, NMS_E_ARG, "variant must be 0, 1 or 2"); c->opt_variant = (int)value; }
-    else if (!strcmp(key, "timing")) c->opt_timing = value != 0;
+    else if (!strcmp(key, "timing")) { c->opt_timing = value != 0; for (Timer& t : c->timers) t.used = 0; }
     else if (!strcmp(key, "chunks")) { if (value < 0) return fail(c, NMS_E_ARG, "chunks must be >= 0"); c->opt_chunks = (int)value; }
     else if (!strcmp(key, "qt")) { if (value != 0 && value != 4 && value != 8 && value != 16) return fail(c, NMS_E_ARG, "qt must be 0, 4, 8 or 16"); c->opt_qt = (int)value; }
     else return fail(c, NMS_E_ARG, "unknown option '%s'", key);
@@ -475,9 +479,25 @@ nms_status nms_kernel_time_ms(nms_ctx* c, nms_timer which, float* ms)
     CHECK_CTX(c);
     if ((int)which < 0 || (int)which >= NMS_T_COUNT || !ms) return fail(c, NMS_E_ARG, "bad timer index or NULL");
     Timer& t = c->timers[which];
-    if (!t.ran) return fail(c, NMS_E_STATE, "that kernel has not run with timing enabled");
-    NMS_CUDA(c, cudaEventSynchronize(t.end));
-    NMS_CUDA(c, cudaEventElapsedTime(ms, t.beg, t.end));
+    if (t.used == 0) return fail(c, NMS_E_STATE, "that kernel has not run with timing enabled");
+    NMS_CUDA(c, cudaEventSynchronize(t.end[t.used - 1]));
+    NMS_CUDA(c, cudaEventElapsedTime(ms, t.beg[t.used - 1], t.end[t.used - 1]));
+    return NMS_OK;
+}
+
+nms_status nms_kernel_time_total(nms_ctx* c, nms_timer which, double* total_ms, int64_t* count)
+{
+    CHECK_CTX(c);
+    if ((int)which < 0 || (int)which >= NMS_T_COUNT || !total_ms || !count) return fail(c, NMS_E_ARG, "bad timer index or NULL");
+    Timer& t = c->timers[which];
+    double sum = 0.0;
+    for (size_t i = 0; i < t.used; ++i) {
+        float ms = 0.f;
+        NMS_CUDA(c, cudaEventSynchronize(t.end[i]));
+        NMS_CUDA(c, cudaEventElapsedTime(&ms, t.beg[i], t.end[i]));
+        sum += (double)ms;
+    }
+    *total_ms = sum; *count = (int64_t)t.used;
     return NMS_OK;
 }
 

@@ -30,9 +30,9 @@ struct TileSrc {           // consumed by the prep kernel
     int32_t particle;      // object index (for centres), -1 if none
 };
 
-struct Timer {
-    cudaEvent_t beg = nullptr, end = nullptr;
-    bool ran = false;
+struct Timer {                         // "timing" option: one CUDA event pair per launch, kept until the next reset
+    std::vector<cudaEvent_t> beg, end;
+    size_t used = 0;                   // pairs recorded since the last reset
 };
 
 struct DevBuf {
