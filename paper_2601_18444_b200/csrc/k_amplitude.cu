@@ -1,37 +1,46 @@
-// k_amplitude.cu -- a-2 (and a-6): the direct sums of Eq. 42-47 (L353-L368) on the FP32 + XU pipes.
+// k_amplitude.cu -- a-2 (and a-6): the direct sums of Eq. 42-47 (L353-L368) on the FP32, FP64 and XU pipes.
 //
 //   A_c(q) = sum_j w_cj exp(-i Psi_j(q)),  Psi_j = q_y Y_j + q_z Z_j  (Eq. 41),  c in {N, x, y, z}.
 //
 // Work decomposition: grid = (detector blocks) x (cell chunks).  A block owns 128*QT detector points
 // (thread = one position along the fast detector index i1 and QT consecutive positions along i0) and
-// walks the tiles of its chunk.  Tiles (<= 1024 cells, 24 B each) are brought into shared memory by one
-// elected thread with cp.async.bulk + mbarrier, double buffered; every lane of a warp reads the same
-// cell (LDS broadcast, no bank conflicts) and updates 8 fp32 accumulators per detector point.
+// walks the tiles of its chunk.  Tiles (<= 512 cells as 256 CellPair records of 64 B) are brought into
+// shared memory by one elected thread with cp.async.bulk + mbarrier, double buffered; every lane of a warp
+// reads the same record (LDS.128 broadcast, no bank conflicts).
 //
-// Numerics: cells are stored relative to a tile origin r0, so the in-tile phase is small and its fp32
-// rounding negligible; because the sum is linear,  sum_j w_j e^{-i q.(r0+d_j)} = e^{-i q.r0} sum_j w_j
-// e^{-i q.d_j}:  at the end of a tile the thread rotates its 8 fp32 tile sums by the tile phasor
-// (phase in fp64, reduced exactly to [-1/2,1/2] cycles) and adds them to fp64 chunk partials in global
-// memory (block-private slots, plain read-modify-write, deterministic).  The epilogue kernel sums the
-// chunks and forms the responses.
+// Arithmetic per (cell, detector point) -- B200 has three independent pipes that all get work:
+//   FP64 pipe : the phase in CYCLES, t = (q/2pi).r, by DFMA with the addend 1.5*2^20: the sum is rounded
+//               to a multiple of 2^-32, so the low mantissa word of the result is frac(t) * 2^32 as a
+//               two's-complement integer in [-1/2, 1/2) cycle, whatever the magnitude of t -- the
+//               "t - rint(t)" reduction of the north star, done by the rounding of the adder, with no fp32
+//               phase rounding and no tile origins;
+//   conversion: one I2FP turns that word into a float (|error| <= 2^-25 cycle = 1.9e-7 rad);
+//   FP32 pipe : packed mul/fma.rn.f32x2 over the two cells of a CellPair: x = 2 pi frac (1 op), then the
+//               8 accumulations w_c cos, w_c sin (4 packed ops per pair);
+//   XU pipe   : sin.approx / cos.approx of x in [-pi, pi) (absolute error 2^-21.4, CUDA C Programming Guide).
+// Accumulators are fp32 over one tile only (<= 256 additions per packed half); at the end of a tile they
+// are added to fp64 chunk partials in global memory (block-private slots, plain read-modify-write,
+// deterministic).  The epilogue kernel sums the chunks and forms the responses.
 //
-// Phasor variants (MODE):
-//   1  general direct : t = q_y dY + q_z dZ per pair, sin/cos by MUFU                     (list grids)
-//   2  polar direct   : p = s dY + c dZ per (cell,thread), t_k = q_k p, MUFU              (any |q| spacing)
-//   4  cart. direct   : u = q_y dY per (cell,thread), t_k = u + q_z,k dZ, MUFU
-//   3  line recurrence: the thread's QT points are equally spaced on a line q_k = b + k s; base and step
-//                       phasors by MUFU once per (cell,thread), then a complex rotation per point
-//                       (4 FP32 ops, no MUFU), resynchronised at every cell.
+// Phase variants (MODE): how t is formed for the thread's QT points
+//   0  polar   : p = sin(th) Y + cos(th) Z per (cell, thread) [2 fp64 ops], t_k = q'_k p + magic [1 per pair]
+//   1  cart.   : u = q'_y Y per (cell, thread) [1], t_k = (q'_z,k Z + u) + magic [2 per pair]
+//   2  list    : t_k = (q'_z,k Z + q'_y,k Y) + magic [3 per pair]
 #include "nms_internal.h"
 #include "nms_response.cuh"
 
 namespace nms {
 
 constexpr int AMP_THREADS = 128;
+constexpr int TILE_PAIRS = TILE / 2;
+
+typedef unsigned long long u64;
+
+constexpr double MAGIC = 1572864.0;                 // 1.5 * 2^20: ulp = 2^-32 (needs |t| < 2^19 cycles)
+constexpr double INV_2PI = 0.15915494309189533577;
 
 struct AmpArgs {
-    const float4* A;
-    const float2* B;
+    const CellPair* cells;
     const TileMeta* tiles;
     const int32_t* chunk_begin;   // [n_chunks+1] or NULL (equal parts of n_tiles)
     int n_tiles;
@@ -76,41 +85,168 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
                      smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
-__device__ __forceinline__ void issue_tile(const AmpArgs& a, int tile, float4* dA, float2* dB, uint64_t* bar)
+__device__ __forceinline__ void issue_tile(const AmpArgs& a, int tile, CellPair* dst, uint64_t* bar)
 {
     const TileMeta tm = a.tiles[tile];
-    const uint32_t n = (uint32_t)tm.n_slots;
+    const uint32_t bytes = (uint32_t)(tm.n_slots / 2) * (uint32_t)sizeof(CellPair);
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-    mbar_expect_tx(bar, n * 24u);
-    bulk_g2s(dA, a.A + tm.first_slot, n * 16u, bar);
-    bulk_g2s(dB, a.B + tm.first_slot, n * 8u, bar);
+    mbar_expect_tx(bar, bytes);
+    bulk_g2s(dst, a.cells + tm.first_slot / 2, bytes, bar);
 }
 
-// 8 accumulate FFMAs of one (cell, detector point) pair: sums of w cos and w sin.
-__device__ __forceinline__ void accumulate(float (&acc)[8], const float4& ca, const float2& cb, float c, float s)
+// ---- packed fp32x2 arithmetic (sm_100 PTX; SASS FFMA2) -------------------------------------------
+__device__ __forceinline__ u64 pack2(float lo, float hi)
 {
-    acc[0] = fmaf(ca.z, c, acc[0]); acc[1] = fmaf(ca.z, s, acc[1]);
-    acc[2] = fmaf(ca.w, c, acc[2]); acc[3] = fmaf(ca.w, s, acc[3]);
-    acc[4] = fmaf(cb.x, c, acc[4]); acc[5] = fmaf(cb.x, s, acc[5]);
-    acc[6] = fmaf(cb.y, c, acc[6]); acc[7] = fmaf(cb.y, s, acc[7]);
+    u64 d;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(d) : "f"(lo), "f"(hi));
+    return d;
+}
+__device__ __forceinline__ void unpack2(u64 v, float& lo, float& hi)
+{
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ u64 ffma2(u64 a, u64 b, u64 c)
+{
+    u64 d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ u64 fmul2(u64 a, u64 b)
+{
+    u64 d;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
 }
 
-template <int MODE, int QT, bool SPLIT, int UNR, int MINB>
-__global__ void __launch_bounds__(AMP_THREADS, MINB) k_amp(const AmpArgs a)
+// The low words of ma, mb hold frac(t) * 2^32 as signed integers (t = phase in cycles, see MAGIC) ->
+// x = 2 pi frac in [-pi, pi), packed.  One I2FP each (24 significant bits: |error| <= 2^-25 cycle) and
+// one packed multiply.
+__device__ __forceinline__ u64 phase_to_x(double ma, double mb)
 {
-    extern __shared__ __align__(128) unsigned char smem_raw[];
-    float4* sA = reinterpret_cast<float4*>(smem_raw);                               // [2][TILE]
-    float2* sB = reinterpret_cast<float2*>(smem_raw + 2 * TILE * sizeof(float4));    // [2][TILE]
-    uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + 2 * TILE * (sizeof(float4) + sizeof(float2)));
+    const float TWO_PI_2M32 = 0x1.921fb6p-30f;   // fl(2 pi) * 2^-32
+    const float fa = __int2float_rn(__double2loint(ma));
+    const float fb = __int2float_rn(__double2loint(mb));
+    return fmul2(pack2(fa, fb), pack2(TWO_PI_2M32, TWO_PI_2M32));
+}
 
-    const int tid = threadIdx.x;
-    const int chunk = blockIdx.y;
-    int tile_beg, tile_end;   // chunk boundaries: a table in split mode (object boundaries), else equal parts
+// 8 accumulations of one (cell pair, detector point): acc[2c] += w_c cos, acc[2c+1] += w_c sin, packed {a, b}
+__device__ __forceinline__ void accumulate(u64 (&acc)[8], const ulonglong2& w01, const ulonglong2& w23, u64 c2, u64 s2)
+{
+    acc[0] = ffma2(w01.x, c2, acc[0]); acc[1] = ffma2(w01.x, s2, acc[1]);
+    acc[2] = ffma2(w01.y, c2, acc[2]); acc[3] = ffma2(w01.y, s2, acc[3]);
+    acc[4] = ffma2(w23.x, c2, acc[4]); acc[5] = ffma2(w23.x, s2, acc[5]);
+    acc[6] = ffma2(w23.y, c2, acc[6]); acc[7] = ffma2(w23.y, s2, acc[7]);
+}
+
+// Add the sums Ap[8] of one tile at detector point f to the fp64 chunk partials (block-private slots, plain
+// read-modify-write).  SPLIT (a-6, Eq. 49-50): ppart carries the running amplitudes of the
+// current object across its tiles; when the object is complete its responses B(A_p, A_p) go to the form
+// accumulators and A_p to the total amplitudes.
+template <bool SPLIT>
+__device__ __forceinline__ void flush_point(const AmpArgs& a, int chunk, int64_t f, double (&Ap)[8], bool first,
+                                            bool p_first, bool p_last, bool first_total)
+{
+    if (!SPLIT) {
+#pragma unroll
+        for (int r = 0; r < 8; ++r) {
+            double* dst = a.part + ((int64_t)chunk * 8 + r) * a.n_q + f;
+            *dst = first ? Ap[r] : (*dst + Ap[r]);
+        }
+    } else {
+#pragma unroll
+        for (int r = 0; r < 8; ++r) {
+            double* pp = a.ppart + ((int64_t)chunk * 8 + r) * a.n_q + f;
+            if (!p_first) Ap[r] += *pp;
+            if (!p_last) *pp = Ap[r];
+        }
+        if (p_last) {
+            const double2 d = a.sc[f];
+            double val[NMS_KIND_COUNT];
+            responses_at_point(Ap, d.x, d.y, a.rp, val);
+            for (int i = 0; i < a.n_kinds; ++i) {
+                double* dst = a.form + ((int64_t)chunk * a.n_kinds + i) * a.n_q + f;
+                const double v = val[a.kinds[i]];
+                *dst = first_total ? v : (*dst + v);
+            }
+#pragma unroll
+            for (int r = 0; r < 8; ++r) {
+                double* dst = a.part + ((int64_t)chunk * 8 + r) * a.n_q + f;
+                *dst = first_total ? Ap[r] : (*dst + Ap[r]);
+            }
+        }
+    }
+}
+
+__device__ __forceinline__ void chunk_range(const AmpArgs& a, int& tile_beg, int& tile_end)
+{
+    const int chunk = blockIdx.y;   // chunk boundaries: a table in split mode (object boundaries), else equal parts
     if (a.chunk_begin) { tile_beg = a.chunk_begin[chunk]; tile_end = a.chunk_begin[chunk + 1]; }
     else {
         tile_beg = (int)(((int64_t)a.n_tiles * chunk) / gridDim.y);
         tile_end = (int)(((int64_t)a.n_tiles * (chunk + 1)) / gridDim.y);
     }
+}
+
+// ---- exact variant: everything in fp64 -----------------------------------------------------------
+// One thread per detector point, cells read straight from global memory (every lane of a block reads the
+// same record: L1 broadcast).  Phase t = (q/2pi).r in fp64, reduced exactly to [-1/2, 1/2] cycle, sincospi
+// and the 8 accumulations in fp64.  ~50 fp64 operations per pair: 7x slower than the fp32 kernels, chosen
+// automatically only for small problems (launch-bound anyway), where it makes the result exact to the
+// fp32 rounding of the rotated weights.  See DESIGN.md section 7 (precision policy).
+template <bool SPLIT>
+__global__ void __launch_bounds__(AMP_THREADS) k_amp_f64(const AmpArgs a)
+{
+    const int chunk = blockIdx.y;
+    int tile_beg, tile_end;
+    chunk_range(a, tile_beg, tile_end);
+    const int64_t f = (int64_t)blockIdx.x * AMP_THREADS + threadIdx.x;
+    if (f >= a.n_q) return;
+    const double2 q = a.qc[f];
+    const double qy = q.x * INV_2PI, qz = q.y * INV_2PI;
+    bool first_total = true;
+    for (int t = tile_beg; t < tile_end; ++t) {
+        const TileMeta tm = a.tiles[t];
+        const CellPair* __restrict__ tC = a.cells + tm.first_slot / 2;
+        double Ap[8];
+#pragma unroll
+        for (int r = 0; r < 8; ++r) Ap[r] = 0.0;
+        const int np = tm.n_slots >> 1;
+        for (int j = 0; j < np; ++j) {
+            const CellPair cp = tC[j];
+#pragma unroll
+            for (int half = 0; half < 2; ++half) {
+                const double Y = half ? cp.Yb : cp.Ya, Z = half ? cp.Zb : cp.Za;
+                double ph = fma(qz, Z, qy * Y);          // Eq. 41, in cycles
+                ph -= rint(ph);
+                double sn, cs;
+                sincospi(2.0 * ph, &sn, &cs);
+                const double w[4] = {(double)(half ? cp.wN.y : cp.wN.x), (double)(half ? cp.wx.y : cp.wx.x),
+                                     (double)(half ? cp.wy.y : cp.wy.x), (double)(half ? cp.wz.y : cp.wz.x)};
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    Ap[2 * c] = fma(w[c], cs, Ap[2 * c]);            // Re: + sum w cos(Psi)   (Eq. 44, 46)
+                    Ap[2 * c + 1] = fma(-w[c], sn, Ap[2 * c + 1]);   // Im: - sum w sin(Psi)   (Eq. 45, 47)
+                }
+            }
+        }
+        const bool p_first = SPLIT ? ((tm.flags & 2) != 0) : false;
+        const bool p_last = SPLIT ? ((tm.flags & 1) != 0) : false;
+        flush_point<SPLIT>(a, chunk, f, Ap, t == tile_beg, p_first, p_last, first_total);
+        if (SPLIT && p_last) first_total = false;
+    }
+}
+
+template <int MODE, int QT, bool SPLIT, int MINB>
+__global__ void __launch_bounds__(AMP_THREADS, MINB) k_amp(const AmpArgs a)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    CellPair* sC = reinterpret_cast<CellPair*>(smem_raw);                                  // [2][TILE_PAIRS]
+    uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + 2 * TILE_PAIRS * sizeof(CellPair));
+
+    const int tid = threadIdx.x;
+    const int chunk = blockIdx.y;
+    int tile_beg, tile_end;
+    chunk_range(a, tile_beg, tile_end);
 
     // ---- this thread's detector points ---------------------------------------------------------
     const int n_groups = (a.n0 + QT - 1) / QT;
@@ -124,31 +260,24 @@ __global__ void __launch_bounds__(AMP_THREADS, MINB) k_amp(const AmpArgs a)
     const int kclamp = max(min(QT, a.n0 - i0), 1);
     const int64_t flat0 = (int64_t)i0 * a.n1 + i1;
 
-    float c0 = 0.f, c1 = 0.f, c2 = 0.f, c3 = 0.f;   // mode-dependent per-thread constants
-    float g[QT], h[QT];                              // per-point constants (modes 1, 2, 4)
-    if (MODE == 1) {
+    // per-thread constants in cycles/nm (q' = q / 2 pi)
+    double c0 = 0.0, c1 = 0.0;     // MODE 0: sin th, cos th;  MODE 1: q'_y
+    double g[QT], h[QT];           // MODE 0: q'_k;  MODE 1: q'_z,k;  MODE 2: q'_y,k and q'_z,k
 #pragma unroll
-        for (int k = 0; k < QT; ++k) {
-            const double2 q = a.qc[flat0 + (int64_t)min(k, kclamp - 1) * a.n1];
-            g[k] = (float)q.x; h[k] = (float)q.y;
+    for (int k = 0; k < QT; ++k) {
+        const int kk = min(k, kclamp - 1);
+        if (MODE == 0) {
+            g[k] = (double)a.u0[i0 + kk] * INV_2PI;
+            h[k] = 0.0;
+        } else {
+            const double2 q = a.qc[flat0 + (int64_t)kk * a.n1];
+            g[k] = q.y * INV_2PI;      // q'_z
+            h[k] = q.x * INV_2PI;      // q'_y
         }
-    } else if (MODE == 2) {
-        const double2 d = a.sc[flat0];
-        c0 = (float)d.x; c1 = (float)d.y;
-#pragma unroll
-        for (int k = 0; k < QT; ++k) g[k] = a.u0[i0 + min(k, kclamp - 1)];
-    } else if (MODE == 4) {
-        c0 = (float)a.qc[flat0].x;
-#pragma unroll
-        for (int k = 0; k < QT; ++k) g[k] = a.u0[i0 + min(k, kclamp - 1)];
-    } else {   // MODE 3
-        const double2 qb = a.qc[flat0];
-        const double2 qe = a.qc[flat0 + (int64_t)(kclamp - 1) * a.n1];
-        const double inv = kclamp > 1 ? 1.0 / (double)(kclamp - 1) : 0.0;
-        c0 = (float)qb.x; c1 = (float)qb.y;
-        c2 = (float)((qe.x - qb.x) * inv); c3 = (float)((qe.y - qb.y) * inv);
     }
-    (void)h;
+    if (MODE == 0) { const double2 d = a.sc[flat0]; c0 = d.x; c1 = d.y; }
+    if (MODE == 1) c0 = h[0];
+    (void)c1;
 
     if (tid == 0) {
         mbar_init(&bar[0], 1);
@@ -157,71 +286,57 @@ __global__ void __launch_bounds__(AMP_THREADS, MINB) k_amp(const AmpArgs a)
     }
     __syncthreads();
     if (tid == 0) {
-        if (tile_beg < tile_end) issue_tile(a, tile_beg, sA, sB, &bar[0]);
-        if (tile_beg + 1 < tile_end) issue_tile(a, tile_beg + 1, sA + TILE, sB + TILE, &bar[1]);
+        if (tile_beg < tile_end) issue_tile(a, tile_beg, sC, &bar[0]);
+        if (tile_beg + 1 < tile_end) issue_tile(a, tile_beg + 1, sC + TILE_PAIRS, &bar[1]);
     }
 
-    float acc[QT][8];
+    u64 acc[QT][8];
     bool first_total = true;   // SPLIT: no object of this chunk has been completed yet
 
     for (int t = tile_beg; t < tile_end; ++t) {
         const int it = t - tile_beg;
         const int stage = it & 1;
         const TileMeta tm = a.tiles[t];
-        const float4* __restrict__ tA = sA + stage * TILE;
-        const float2* __restrict__ tB = sB + stage * TILE;
+        const CellPair* __restrict__ tC = sC + stage * TILE_PAIRS;
 #pragma unroll
         for (int k = 0; k < QT; ++k)
 #pragma unroll
-            for (int r = 0; r < 8; ++r) acc[k][r] = 0.f;
+            for (int r = 0; r < 8; ++r) acc[k][r] = 0ull;
         mbar_wait(&bar[stage], (uint32_t)((it >> 1) & 1));
 
-        const int n = tm.n_slots;
-#pragma unroll UNR
-        for (int j = 0; j < n; ++j) {
-            const float4 ca = tA[j];
-            const float2 cb = tB[j];
-            if (MODE == 1) {
+        const int np = tm.n_slots >> 1;
+#pragma unroll 1
+        for (int j = 0; j < np; ++j) {
+            const double2 Y = *reinterpret_cast<const double2*>(&tC[j].Ya);
+            const double2 Z = *reinterpret_cast<const double2*>(&tC[j].Za);
+            const ulonglong2 w01 = *reinterpret_cast<const ulonglong2*>(&tC[j].wN);
+            const ulonglong2 w23 = *reinterpret_cast<const ulonglong2*>(&tC[j].wy);
+            double pa = 0.0, pb = 0.0;
+            if (MODE == 0) { pa = fma(c1, Z.x, c0 * Y.x); pb = fma(c1, Z.y, c0 * Y.y); }   // Eq. 41 / q
+            if (MODE == 1) { pa = c0 * Y.x; pb = c0 * Y.y; }
+            u64 x2[QT];
 #pragma unroll
-                for (int k = 0; k < QT; ++k) {
-                    const float ph = fmaf(h[k], ca.y, g[k] * ca.x);
-                    accumulate(acc[k], ca, cb, __cosf(ph), __sinf(ph));
-                }
-            } else if (MODE == 2) {
-                const float p = fmaf(c1, ca.y, c0 * ca.x);
+            for (int k = 0; k < QT; ++k) {
+                double ma, mb;
+                if (MODE == 0) { ma = fma(g[k], pa, MAGIC); mb = fma(g[k], pb, MAGIC); }
+                else if (MODE == 1) { ma = fma(g[k], Z.x, pa) + MAGIC; mb = fma(g[k], Z.y, pb) + MAGIC; }
+                else { ma = fma(g[k], Z.x, h[k] * Y.x) + MAGIC; mb = fma(g[k], Z.y, h[k] * Y.y) + MAGIC; }
+                x2[k] = phase_to_x(ma, mb);
+            }
 #pragma unroll
-                for (int k = 0; k < QT; ++k) {
-                    const float ph = g[k] * p;
-                    accumulate(acc[k], ca, cb, __cosf(ph), __sinf(ph));
-                }
-            } else if (MODE == 4) {
-                const float u = c0 * ca.x;
-#pragma unroll
-                for (int k = 0; k < QT; ++k) {
-                    const float ph = fmaf(g[k], ca.y, u);
-                    accumulate(acc[k], ca, cb, __cosf(ph), __sinf(ph));
-                }
-            } else {
-                const float t0 = fmaf(c1, ca.y, c0 * ca.x);
-                const float dt = fmaf(c3, ca.y, c2 * ca.x);
-                float pc = __cosf(t0), ps = __sinf(t0);
-                const float dc = __cosf(dt), ds = __sinf(dt);
-#pragma unroll
-                for (int k = 0; k < QT; ++k) {
-                    accumulate(acc[k], ca, cb, pc, ps);
-                    if (k < QT - 1) {
-                        const float nc = fmaf(pc, dc, -(ps * ds));
-                        const float ns = fmaf(ps, dc, pc * ds);
-                        pc = nc; ps = ns;
-                    }
-                }
+            for (int k = 0; k < QT; ++k) {
+                float xa, xb;
+                unpack2(x2[k], xa, xb);
+                const u64 c2 = pack2(__cosf(xa), __cosf(xb));
+                const u64 s2 = pack2(__sinf(xa), __sinf(xb));
+                accumulate(acc[k], w01, w23, c2, s2);
             }
         }
 
         __syncthreads();   // every thread is done with this stage: refill it while the flush runs
-        if (tid == 0 && t + 2 < tile_end) issue_tile(a, t + 2, sA + stage * TILE, sB + stage * TILE, &bar[stage]);
+        if (tid == 0 && t + 2 < tile_end) issue_tile(a, t + 2, sC + stage * TILE_PAIRS, &bar[stage]);
 
-        // ---- flush: rotate the tile sums by exp(-i q.r0) and add them to the fp64 chunk partials --
+        // ---- flush: add the fp32 tile sums to the fp64 chunk partials -----------------------------
         const bool first = (t == tile_beg);
         const bool p_first = SPLIT ? ((tm.flags & 2) != 0) : false;
         const bool p_last = SPLIT ? ((tm.flags & 1) != 0) : false;
@@ -229,52 +344,16 @@ __global__ void __launch_bounds__(AMP_THREADS, MINB) k_amp(const AmpArgs a)
         for (int k = 0; k < QT; ++k) {
             if (k < kmax) {
                 const int64_t f = flat0 + (int64_t)k * a.n1;
-                const double2 q = a.qc[f];
-                double ph = (q.x * tm.Y0 + q.y * tm.Z0) * 0.15915494309189533577;   // cycles
-                ph -= rint(ph);
-                const float rh = (float)ph;
-                const float rl = (float)(ph - (double)rh);
-                float s0f, c0f;
-                sincospif(2.0f * rh, &s0f, &c0f);
-                const double e = 6.283185307179586 * (double)rl;
-                const double cd = (double)c0f - e * (double)s0f;
-                const double sd = (double)s0f + e * (double)c0f;
                 double Ap[8];
 #pragma unroll
                 for (int w = 0; w < 4; ++w) {
-                    const double C = (double)acc[k][2 * w], S = (double)acc[k][2 * w + 1];
-                    Ap[2 * w] = C * cd - S * sd;          // Re: + sum w cos(Psi)   (Eq. 44, 46)
-                    Ap[2 * w + 1] = -(S * cd + C * sd);   // Im: - sum w sin(Psi)   (Eq. 45, 47)
+                    float ca, cb, sa, sb;
+                    unpack2(acc[k][2 * w], ca, cb);
+                    unpack2(acc[k][2 * w + 1], sa, sb);
+                    Ap[2 * w] = (double)ca + (double)cb;          // Re: + sum w cos(Psi)   (Eq. 44, 46)
+                    Ap[2 * w + 1] = -((double)sa + (double)sb);   // Im: - sum w sin(Psi)   (Eq. 45, 47)
                 }
-                if (!SPLIT) {
-#pragma unroll
-                    for (int r = 0; r < 8; ++r) {
-                        double* dst = a.part + ((int64_t)chunk * 8 + r) * a.n_q + f;
-                        *dst = first ? Ap[r] : (*dst + Ap[r]);
-                    }
-                } else {
-#pragma unroll
-                    for (int r = 0; r < 8; ++r) {
-                        double* pp = a.ppart + ((int64_t)chunk * 8 + r) * a.n_q + f;
-                        if (!p_first) Ap[r] += *pp;
-                        if (!p_last) *pp = Ap[r];
-                    }
-                    if (p_last) {   // object complete: form += B(A_p, A_p), total amplitude += A_p  (Eq. 49-50)
-                        const double2 d = a.sc[f];
-                        double val[NMS_KIND_COUNT];
-                        responses_at_point(Ap, d.x, d.y, a.rp, val);
-                        for (int i = 0; i < a.n_kinds; ++i) {
-                            double* dst = a.form + ((int64_t)chunk * a.n_kinds + i) * a.n_q + f;
-                            const double v = val[a.kinds[i]];
-                            *dst = first_total ? v : (*dst + v);
-                        }
-#pragma unroll
-                        for (int r = 0; r < 8; ++r) {
-                            double* dst = a.part + ((int64_t)chunk * 8 + r) * a.n_q + f;
-                            *dst = first_total ? Ap[r] : (*dst + Ap[r]);
-                        }
-                    }
-                }
+                flush_point<SPLIT>(a, chunk, f, Ap, first, p_first, p_last, first_total);
             }
         }
         if (SPLIT && p_last) first_total = false;
@@ -282,30 +361,28 @@ __global__ void __launch_bounds__(AMP_THREADS, MINB) k_amp(const AmpArgs a)
 }
 
 // ---- host side: planning and dispatch ------------------------------------------------------------
-constexpr size_t AMP_SMEM = 2 * TILE * (sizeof(float4) + sizeof(float2)) + 2 * sizeof(uint64_t);
+constexpr size_t AMP_SMEM = 2 * TILE_PAIRS * sizeof(CellPair) + 2 * sizeof(uint64_t);
 
 typedef void (*amp_kernel_t)(const AmpArgs);
 
-template <int MODE, int QT, int UNR, int MINB>
+template <int MODE, int QT, int MINB>
 static amp_kernel_t pick_split(bool split)
 {
-    return split ? (amp_kernel_t)k_amp<MODE, QT, true, UNR, MINB> : (amp_kernel_t)k_amp<MODE, QT, false, UNR, MINB>;
+    return split ? (amp_kernel_t)k_amp<MODE, QT, true, MINB> : (amp_kernel_t)k_amp<MODE, QT, false, MINB>;
 }
 
+// variant: 1 list direct, 2 polar direct, 4 cartesian direct (fp32 accumulation), 8 exact (fp64)
 static amp_kernel_t pick_kernel(int variant, int qt, bool split)
 {
     switch (variant) {
-    case 1: return pick_split<1, 4, 2, 4>(split);
+    case 1: return pick_split<2, 4, 3>(split);
     case 2:
-        if (qt == 4) return pick_split<2, 4, 2, 4>(split);
-        return pick_split<2, 8, 2, 4>(split);
+        if (qt == 4) return pick_split<0, 4, 3>(split);
+        return pick_split<0, 8, 2>(split);
     case 4:
-        if (qt == 4) return pick_split<4, 4, 2, 4>(split);
-        return pick_split<4, 8, 2, 4>(split);
-    default:
-        if (qt == 4) return pick_split<3, 4, 2, 4>(split);
-        if (qt == 8) return pick_split<3, 8, 2, 4>(split);
-        return pick_split<3, 16, 1, 2>(split);
+        if (qt == 4) return pick_split<1, 4, 3>(split);
+        return pick_split<1, 8, 2>(split);
+    default: return split ? (amp_kernel_t)k_amp_f64<true> : (amp_kernel_t)k_amp_f64<false>;
     }
 }
 
@@ -313,24 +390,25 @@ static int64_t ceil_div(int64_t a, int64_t b) { return (a + b - 1) / b; }
 
 nms_status plan_amplitude(nms_ctx* c, bool split, AmpPlan* plan)
 {
-    // variant: list grids are general; equally spaced lines allow the recurrence; otherwise line-direct
+    // precision policy: small problems run the exact fp64 kernel
     int variant;
-    if (c->g_type == 2) variant = 1;
-    else if (c->g_uniform && c->opt_variant != 1) variant = 3;
+    const bool small = (double)c->W * (double)c->n_q <= 1073741824.0;
+    if (c->opt_variant == 3 || (c->opt_variant == 0 && small)) variant = 8;
+    else if (c->g_type == 2) variant = 1;
     else variant = (c->g_type == 0) ? 2 : 4;
-    if (c->opt_variant == 2 && variant != 3 && c->g_type != 2)
-        return fail(c, NMS_E_UNSUPPORTED, "recurrence variant forced but the detector lines are not equally spaced");
+    if (c->opt_variant == 2)
+        return fail(c, NMS_E_UNSUPPORTED, "the line-recurrence variant is not available for this detector / sample");
 
     // units of work along the cell dimension: tiles, or whole objects in split mode
     const int64_t units = split ? c->K : c->n_tiles;
-    int dev_slots_guess = c->sm_count * 4;
+    int dev_slots_guess = c->sm_count * 3;
     // q points per thread: the largest that still yields enough blocks to fill the device
     int qt_opts[3]; int n_opts = 0;
-    if (variant == 1) { qt_opts[n_opts++] = 4; }
-    else if (variant == 3) { qt_opts[n_opts++] = 16; qt_opts[n_opts++] = 8; qt_opts[n_opts++] = 4; }
+    if (variant == 8) { qt_opts[n_opts++] = 1; }
+    else if (variant == 1) { qt_opts[n_opts++] = 4; }
     else { qt_opts[n_opts++] = 8; qt_opts[n_opts++] = 4; }
     int qt = qt_opts[n_opts - 1];
-    if (c->opt_qt) {
+    if (c->opt_qt && variant != 8) {
         bool ok = false;
         for (int i = 0; i < n_opts; ++i) ok |= (qt_opts[i] == c->opt_qt);
         if (!ok) return fail(c, NMS_E_ARG, "option qt=%d is not available for kernel variant %d", c->opt_qt, variant);
@@ -341,13 +419,15 @@ nms_status plan_amplitude(nms_ctx* c, bool split, AmpPlan* plan)
             if (qb * units >= dev_slots_guess || i == n_opts - 1) { qt = qt_opts[i]; break; }
         }
     }
+    const size_t smem = variant == 8 ? 0 : AMP_SMEM;
     amp_kernel_t kern = pick_kernel(variant, qt, split);
     NMS_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)AMP_SMEM));
     int occ = 0;
-    NMS_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, AMP_THREADS, AMP_SMEM));
+    NMS_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, AMP_THREADS, smem));
     if (occ < 1) return fail(c, NMS_E_CUDA, "amplitude kernel does not fit on an SM");
     const int64_t slots = (int64_t)c->sm_count * occ;
-    const int64_t n_qb = ceil_div(ceil_div(c->g_n0, qt) * c->g_n1, AMP_THREADS);
+    const int64_t n_qb = variant == 8 ? ceil_div(c->n_q, AMP_THREADS)
+                                      : ceil_div(ceil_div(c->g_n0, qt) * c->g_n1, AMP_THREADS);
 
     // number of cell chunks: smallest count whose last wave is >= 97 % full (equal-sized blocks)
     int64_t max_chunks = units;
@@ -401,7 +481,7 @@ nms_status launch_amplitude(nms_ctx* c, const AmpPlan& plan, const int32_t* kind
         if (nms_status st = ensure(c, c->formpart, sizeof(double) * (size_t)n_kinds * (size_t)c->n_q * n_chunks)) return st;
     }
     AmpArgs a;
-    a.A = (const float4*)c->cellA.p; a.B = (const float2*)c->cellB.p;
+    a.cells = (const CellPair*)c->cells.p;
     a.tiles = (const TileMeta*)c->tile_meta.p;
     a.chunk_begin = plan.split ? (const int32_t*)c->chunk_begin.p : nullptr;
     a.n_tiles = (int)c->n_tiles;
@@ -415,7 +495,7 @@ nms_status launch_amplitude(nms_ctx* c, const AmpPlan& plan, const int32_t* kind
     NMS_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)AMP_SMEM));
     dim3 grid((unsigned)plan.n_qblocks, (unsigned)n_chunks);
     timer_begin(c, NMS_T_AMPLITUDE);
-    kern<<<grid, AMP_THREADS, AMP_SMEM, c->stream>>>(a);
+    kern<<<grid, AMP_THREADS, plan.variant == 8 ? 0 : AMP_SMEM, c->stream>>>(a);
     timer_end(c, NMS_T_AMPLITUDE);
     c->launches += 1;
     NMS_CUDA(c, cudaGetLastError());

@@ -1,9 +1,10 @@
 // k_prep.cu -- a-1: rotate + pack the real-space sample into tiles, and detector set-up.
 //
 //  prep kernel   (Eq. 37-41):  r' = R (x + r^k), m' = R m in fp64; only Y, Z (rows 2, 3 of R)
-//                are kept because q_x = 0 on the detector (Eq. 41).  One block per tile: it finds the
-//                tile's bounding-box midpoint (Y0, Z0), stores cells relative to it (one rounding to
-//                fp32) and accumulates sum_j |w_cj| for the tolerance denominators.
+//                are kept because q_x = 0 on the detector (Eq. 41).  One block per tile, one thread per
+//                cell pair: it writes the CellPair record (fp64 Y, Z; weights rounded once to fp32), finds
+//                the tile's bounding-box midpoint (Y0, Z0) and extent, and accumulates sum_j |w_cj| for
+//                the tolerance denominators.
 //  qsetup kernel (Eq. 6): per detector point (q_y, q_z) in fp64 [rad/nm] and
 //                (sin th, cos th) for the response epilogue.
 #include "nms_internal.h"
@@ -22,8 +23,7 @@ struct PrepArgs {
     const int64_t* first_slot;
     const int32_t* flags;
     TileMeta* meta;
-    float4* A;
-    float2* B;
+    CellPair* cells;
     double* wsum;
     double R[9];
 };
@@ -47,7 +47,6 @@ __device__ __forceinline__ double warp_sum(double v)
 __global__ void __launch_bounds__(PREP_THREADS) k_prep(const PrepArgs a)
 {
     __shared__ double red[8][PREP_THREADS / 32];
-    __shared__ double origin[2];
     const int tile = blockIdx.x;
     const TileSrc ts = a.src[tile];
     const int64_t first_slot = a.first_slot[tile];
@@ -66,7 +65,7 @@ __global__ void __launch_bounds__(PREP_THREADS) k_prep(const PrepArgs a)
     double sN = 0.0, sx = 0.0, sy = 0.0, sz = 0.0;
 #pragma unroll
     for (int u = 0; u < PREP_PER_THREAD; ++u) {
-        const int i = tid + u * PREP_THREADS;
+        const int i = 2 * tid + u;
         Y[u] = Z[u] = 0.0;
         wN[u] = wx[u] = wy[u] = wz[u] = 0.f;
         if (i < ts.n_src) {
@@ -106,30 +105,20 @@ __global__ void __launch_bounds__(PREP_THREADS) k_prep(const PrepArgs a)
         }
         const double Y0 = ts.n_src > 0 ? 0.5 * (v[0] + v[1]) : 0.0;
         const double Z0 = ts.n_src > 0 ? 0.5 * (v[2] + v[3]) : 0.0;
-        origin[0] = Y0; origin[1] = Z0;
         TileMeta tm;
         tm.Y0 = Y0; tm.Z0 = Z0; tm.first_slot = first_slot; tm.n_slots = n_slots; tm.flags = a.flags[tile];
+        tm.ext = ts.n_src > 0 ? (float)fmax(0.5 * (v[1] - v[0]), 0.5 * (v[3] - v[2])) : 0.f;
+        tm.pad_ = 0;
         a.meta[tile] = tm;
         for (int r = 0; r < 4; ++r)
             if (v[4 + r] != 0.0) atomicAdd(a.wsum + r, v[4 + r]);
     }
-    __syncthreads();
-    const double Y0 = origin[0], Z0 = origin[1];
-#pragma unroll
-    for (int u = 0; u < PREP_PER_THREAD; ++u) {
-        const int i = tid + u * PREP_THREADS;
-        if (i < n_slots) {
-            float4 va; float2 vb;
-            if (i < ts.n_src) {
-                va = make_float4((float)(Y[u] - Y0), (float)(Z[u] - Z0), wN[u], wx[u]);
-                vb = make_float2(wy[u], wz[u]);
-            } else {
-                va = make_float4(0.f, 0.f, 0.f, 0.f);
-                vb = make_float2(0.f, 0.f);
-            }
-            a.A[first_slot + i] = va;
-            a.B[first_slot + i] = vb;
-        }
+    if (2 * tid < n_slots) {   // cells beyond n_src are the zero-weight padding (Y = Z = 0, w = 0)
+        CellPair cp;
+        cp.Ya = Y[0]; cp.Yb = Y[1]; cp.Za = Z[0]; cp.Zb = Z[1];
+        cp.wN = make_float2(wN[0], wN[1]); cp.wx = make_float2(wx[0], wx[1]);
+        cp.wy = make_float2(wy[0], wy[1]); cp.wz = make_float2(wz[0], wz[1]);
+        a.cells[first_slot / 2 + tid] = cp;
     }
 }
 
@@ -146,8 +135,7 @@ nms_status launch_prep(nms_ctx* c)
     a.first_slot = (const int64_t*)base;
     a.flags = (const int32_t*)(base + sizeof(int64_t) * (size_t)c->n_tiles);
     a.meta = (TileMeta*)c->tile_meta.p;
-    a.A = (float4*)c->cellA.p;
-    a.B = (float2*)c->cellB.p;
+    a.cells = (CellPair*)c->cells.p;
     a.wsum = (double*)c->wsum.p;
     for (int i = 0; i < 9; ++i) a.R[i] = c->R[i];
     NMS_CUDA(c, cudaMemsetAsync(c->wsum.p, 0, 4 * sizeof(double), c->stream));

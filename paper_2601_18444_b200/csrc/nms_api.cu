@@ -105,8 +105,7 @@ static nms_status build_tiles(nms_ctx* c)
     const size_t bytes = n * (sizeof(TileSrc) + sizeof(int64_t) + sizeof(int32_t));
     if (nms_status st = ensure(c, c->tile_src, bytes)) return st;
     if (nms_status st = ensure(c, c->tile_meta, n * sizeof(TileMeta))) return st;
-    if (nms_status st = ensure(c, c->cellA, (size_t)slot * sizeof(float4))) return st;
-    if (nms_status st = ensure(c, c->cellB, (size_t)slot * sizeof(float2))) return st;
+    if (nms_status st = ensure(c, c->cells, (size_t)(slot / 2) * sizeof(CellPair))) return st;
     if (nms_status st = ensure(c, c->wsum, 4 * sizeof(double))) return st;
     char* base = (char*)c->tile_src.p;
     NMS_CUDA(c, cudaMemcpyAsync(base, c->h_tile_src.data(), n * sizeof(TileSrc), cudaMemcpyHostToDevice, c->stream));
@@ -240,7 +239,7 @@ void nms_destroy(nms_ctx* c)
     if (!c) return;
     cudaSetDevice(c->device);
     cudaStreamSynchronize(c->stream);
-    DevBuf* bufs[] = {&c->raw_pos, &c->raw_N, &c->raw_m, &c->centres, &c->tile_src, &c->tile_meta, &c->cellA, &c->cellB,
+    DevBuf* bufs[] = {&c->raw_pos, &c->raw_N, &c->raw_m, &c->centres, &c->tile_src, &c->tile_meta, &c->cells,
                       &c->wsum, &c->u0, &c->u1, &c->qc, &c->sc, &c->amp64, &c->part, &c->ppart, &c->formpart,
                       &c->chunk_begin, &c->kinds_dev, &c->bin_idx, &c->bin_sum, &c->bin_cnt};
     for (DevBuf* b : bufs) free_buf(*b);
@@ -450,7 +449,7 @@ nms_status nms_set_option(nms_ctx* c, const char* key, int64_t value)
 {
     CHECK_CTX(c);
     if (!key) return fail(c, NMS_E_ARG, "key is NULL");
-    if (!strcmp(key, "variant")) { if (value < 0 || value > 2) return fail(c, NMS_E_ARG, "variant must be 0, 1 or 2"); c->opt_variant = (int)value; }
+    if (!strcmp(key, "variant")) { if (value < 0 || value > 3) return fail(c, NMS_E_ARG, "variant must be 0, 1, 2 or 3"); c->opt_variant = (int)value; }
     else if (!strcmp(key, "timing")) { c->opt_timing = value != 0; for (Timer& t : c->timers) t.used = 0; }
     else if (!strcmp(key, "chunks")) { if (value < 0) return fail(c, NMS_E_ARG, "chunks must be >= 0"); c->opt_chunks = (int)value; }
     else if (!strcmp(key, "qt")) { if (value != 0 && value != 4 && value != 8 && value != 16) return fail(c, NMS_E_ARG, "qt must be 0, 4, 8 or 16"); c->opt_qt = (int)value; }

@@ -10,19 +10,28 @@ namespace nms {
 
 // ---- packed real-space layout (a-1) ----------------------------------------------------------
 // Cells are grouped into tiles of at most TILE consecutive cells (never straddling an object when
-// an object structure is set).  Each tile carries a local origin (Y0,Z0) in fp64; a cell stores its
-// rotated detector-plane coordinates RELATIVE to that origin (Eq. 39-40 minus origin) and its
-// weights:  A[slot] = (dY, dZ, N, m'x),  B[slot] = (m'y, m'z).   X is never needed: q_x = 0 (Eq. 41).
-// Tiles are padded to a multiple of 8 slots with zero-weight cells so that every bulk copy is
-// 16-byte aligned and the inner loop can be unrolled without a tail.
-constexpr int TILE = 1024;
-constexpr int SLOT_PAD = 8;
+// an object structure is set).  A tile is stored as CellPair records: two consecutive cells (a, b)
+// side by side, so that every FP32 operation of the amplitude kernel is a packed fma.rn.f32x2 over the
+// pair.  Coordinates are the rotated detector-plane coordinates Y, Z (Eq. 39-40) in fp64 -- the phase
+// is formed in fp64 (one DFMA per pair on the FP64 pipe), see k_amplitude.cu; X is never needed:
+// q_x = 0 (Eq. 41).  Weights are rounded once to fp32.  Odd tiles are padded with a zero-weight cell.
+constexpr int TILE = 512;
+constexpr int SLOT_PAD = 2;
+
+struct CellPair {          // 64 B, the unit of the bulk copies (16-byte aligned)
+    double Ya, Yb;         // [nm]
+    double Za, Zb;
+    float2 wN, wx;         // {a, b}: nuclear weight, m'_x
+    float2 wy, wz;         // {a, b}: m'_y, m'_z
+};
 
 struct TileMeta {          // consumed by the amplitude kernel
-    double Y0, Z0;         // local origin [nm]
-    int64_t first_slot;    // index into A/B
+    double Y0, Z0;         // bounding-box midpoint [nm] (origin of the line-recurrence kernel)
+    int64_t first_slot;    // index into the cell array (cells, always even)
     int32_t n_slots;       // padded cell count (multiple of SLOT_PAD)
-    int32_t flags;         // bit 0: last tile of its object (form-factor split)
+    int32_t flags;         // bit 0: last tile of its object, bit 1: first tile (form-factor split)
+    float ext;             // max over the tile's cells of |Y - Y0|, |Z - Z0| [nm]
+    int32_t pad_;
 };
 struct TileSrc {           // consumed by the prep kernel
     int64_t src_first;     // first source cell
@@ -73,7 +82,7 @@ struct nms_ctx {
     std::vector<nms::TileSrc> h_tile_src;
     std::vector<int32_t> h_tile_flags;
     std::vector<int64_t> h_tile_first_slot;
-    nms::DevBuf tile_src, tile_meta, cellA, cellB, wsum;   // wsum: double[4]
+    nms::DevBuf tile_src, tile_meta, cells, wsum;   // cells: CellPair[n_slots/2]; wsum: double[4]
 
     // current detector grid
     bool grid_valid = false;
