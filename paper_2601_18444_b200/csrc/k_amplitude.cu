@@ -26,6 +26,20 @@
 //   0  polar   : p = sin(th) Y + cos(th) Z per (cell, thread) [2 fp64 ops], t_k = q'_k p + magic [1 per pair]
 //   1  cart.   : u = q'_y Y per (cell, thread) [1], t_k = (q'_z,k Z + u) + magic [2 per pair]
 //   2  list    : t_k = (q'_z,k Z + q'_y,k Y) + magic [3 per pair]
+//
+// Line recurrence (NB > 0; north star (b): "advanced by a complex-rotation recurrence ... with periodic
+// resync").  The direct path is bound by the XU pipe (2 MUFU per pair at 16 lanes/clk/SM = 8 pairs/clk/SM).
+// Where the abscissa along the thread's line is equally spaced (u0[k] = u0[0] + k d: |q| of a polar grid,
+// q_z of a Cartesian one) the phases of a thread's QT points form an arithmetic progression with the step
+// d' * p (polar) or d' * Z (Cartesian) per cell.  The QT points are cut into NB segments; the phasor of one
+// point per segment (its "base") is evaluated exactly as above -- the resync, at EVERY cell -- and the
+// others are reached from it by at most ceil((QT/NB - 1)/2) complex rotations with the step phasor
+// (cos, sin of the exactly reduced step phase, one evaluation per cell and thread), forwards or backwards
+// (conjugate step).  A rotation is 2 packed multiplies + 2 packed FMAs per cell pair, so a pair costs
+// 12 FP32 lane-operations and the MUFU load drops from 2 to (NB + 1) * 2 / QT per pair.  Error: a point
+// s steps from its base carries (s + 1) MUFU errors (2^-21.4 each) and s fp32 roundings, and the deviation
+// of the fp32 abscissae from the exact progression (<= 1 ulp of q, checked on the host) enters as a phase
+// error <= ulp(q) * |r|; both are measured against the oracle in tests/test_gpu_parity.py.
 #include "nms_internal.h"
 #include "nms_response.cuh"
 
@@ -47,6 +61,7 @@ struct AmpArgs {
     int type, n0, n1;
     int64_t n_q;
     const float* u0;
+    double dq;           // recurrence kernels: spacing of u0 [rad/nm] (fp64, (u0[n0-1] - u0[0]) / (n0 - 1))
     const double2* qc;   // (q_y, q_z) [rad/nm] fp64
     const double2* sc;   // (sin th, cos th)
     double* part;        // [n_chunks][8][n_q]
@@ -236,9 +251,28 @@ __global__ void __launch_bounds__(AMP_THREADS) k_amp_f64(const AmpArgs a)
     }
 }
 
-template <int MODE, int QT, bool SPLIT, int MINB>
+// phasor of the exactly reduced phases (ma, mb) of the two cells of a pair: packed cos and sin
+__device__ __forceinline__ void phasor2(double ma, double mb, u64& c2, u64& s2)
+{
+    float xa, xb;
+    unpack2(phase_to_x(ma, mb), xa, xb);
+    c2 = pack2(__cosf(xa), __cosf(xb));
+    s2 = pack2(__sinf(xa), __sinf(xb));
+}
+
+// (c, s) -> (c cd - s sd, s cd + c sd): advance the phase by the step whose phasor is (cd, sd); nsd = -sd.
+// The backward rotation passes (cd, nsd, sd).
+__device__ __forceinline__ void rotate2(u64 c, u64 s, u64 cd, u64 sd, u64 nsd, u64& co, u64& so)
+{
+    co = ffma2(c, cd, fmul2(s, nsd));
+    so = ffma2(c, sd, fmul2(s, cd));
+}
+
+// NB = 0: direct evaluation of every pair; NB > 0: line recurrence with NB exactly evaluated points per QT
+template <int MODE, int QT, bool SPLIT, int MINB, int NB>
 __global__ void __launch_bounds__(AMP_THREADS, MINB) k_amp(const AmpArgs a)
 {
+    static_assert(NB == 0 || (MODE != 2 && NB <= QT), "the recurrence needs a line of equally spaced abscissae");
     extern __shared__ __align__(128) unsigned char smem_raw[];
     CellPair* sC = reinterpret_cast<CellPair*>(smem_raw);                                  // [2][TILE_PAIRS]
     uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + 2 * TILE_PAIRS * sizeof(CellPair));
@@ -278,6 +312,12 @@ __global__ void __launch_bounds__(AMP_THREADS, MINB) k_amp(const AmpArgs a)
     if (MODE == 0) { const double2 d = a.sc[flat0]; c0 = d.x; c1 = d.y; }
     if (MODE == 1) c0 = h[0];
     (void)c1;
+    const double dq = a.dq * INV_2PI;   // recurrence: spacing of the line in cycles/nm
+    if (NB > 0) {                       // points beyond the detector edge continue the progression (never stored)
+#pragma unroll
+        for (int k = 1; k < QT; ++k)
+            if (k >= kclamp) g[k] += (double)(k - (kclamp - 1)) * dq;   // g[k] was clamped to g[kclamp - 1]
+    }
 
     if (tid == 0) {
         mbar_init(&bar[0], 1);
@@ -314,22 +354,51 @@ __global__ void __launch_bounds__(AMP_THREADS, MINB) k_amp(const AmpArgs a)
             double pa = 0.0, pb = 0.0;
             if (MODE == 0) { pa = fma(c1, Z.x, c0 * Y.x); pb = fma(c1, Z.y, c0 * Y.y); }   // Eq. 41 / q
             if (MODE == 1) { pa = c0 * Y.x; pb = c0 * Y.y; }
-            u64 x2[QT];
+            if (NB == 0) {
+                u64 x2[QT];
 #pragma unroll
-            for (int k = 0; k < QT; ++k) {
-                double ma, mb;
-                if (MODE == 0) { ma = fma(g[k], pa, MAGIC); mb = fma(g[k], pb, MAGIC); }
-                else if (MODE == 1) { ma = fma(g[k], Z.x, pa) + MAGIC; mb = fma(g[k], Z.y, pb) + MAGIC; }
-                else { ma = fma(g[k], Z.x, h[k] * Y.x) + MAGIC; mb = fma(g[k], Z.y, h[k] * Y.y) + MAGIC; }
-                x2[k] = phase_to_x(ma, mb);
-            }
+                for (int k = 0; k < QT; ++k) {
+                    double ma, mb;
+                    if (MODE == 0) { ma = fma(g[k], pa, MAGIC); mb = fma(g[k], pb, MAGIC); }
+                    else if (MODE == 1) { ma = fma(g[k], Z.x, pa) + MAGIC; mb = fma(g[k], Z.y, pb) + MAGIC; }
+                    else { ma = fma(g[k], Z.x, h[k] * Y.x) + MAGIC; mb = fma(g[k], Z.y, h[k] * Y.y) + MAGIC; }
+                    x2[k] = phase_to_x(ma, mb);
+                }
 #pragma unroll
-            for (int k = 0; k < QT; ++k) {
-                float xa, xb;
-                unpack2(x2[k], xa, xb);
-                const u64 c2 = pack2(__cosf(xa), __cosf(xb));
-                const u64 s2 = pack2(__sinf(xa), __sinf(xb));
-                accumulate(acc[k], w01, w23, c2, s2);
+                for (int k = 0; k < QT; ++k) {
+                    float xa, xb;
+                    unpack2(x2[k], xa, xb);
+                    const u64 c2 = pack2(__cosf(xa), __cosf(xb));
+                    const u64 s2 = pack2(__sinf(xa), __sinf(xb));
+                    accumulate(acc[k], w01, w23, c2, s2);
+                }
+            } else {
+                // step phasor of this cell pair: phase step dq' p (polar) or dq' Z (Cartesian), exactly reduced
+                u64 cd, sd;
+                if (MODE == 0) phasor2(fma(dq, pa, MAGIC), fma(dq, pb, MAGIC), cd, sd);
+                else           phasor2(fma(dq, Z.x, MAGIC), fma(dq, Z.y, MAGIC), cd, sd);
+                const u64 nsd = sd ^ 0x8000000080000000ull;
+#pragma unroll
+                for (int b = 0; b < NB; ++b) {
+                    const int lo = (b * QT) / NB, hi = ((b + 1) * QT) / NB - 1;   // segment [lo, hi]
+                    const int kb = lo + (hi - lo + 1) / 2;                         // its exactly evaluated point
+                    u64 cb, sb;
+                    if (MODE == 0) phasor2(fma(g[kb], pa, MAGIC), fma(g[kb], pb, MAGIC), cb, sb);
+                    else           phasor2(fma(g[kb], Z.x, pa) + MAGIC, fma(g[kb], Z.y, pb) + MAGIC, cb, sb);
+                    accumulate(acc[kb], w01, w23, cb, sb);
+                    u64 c = cb, s = sb;
+#pragma unroll
+                    for (int k = kb + 1; k <= hi; ++k) {
+                        rotate2(c, s, cd, sd, nsd, c, s);
+                        accumulate(acc[k], w01, w23, c, s);
+                    }
+                    c = cb; s = sb;
+#pragma unroll
+                    for (int k = kb - 1; k >= lo; --k) {
+                        rotate2(c, s, cd, nsd, sd, c, s);
+                        accumulate(acc[k], w01, w23, c, s);
+                    }
+                }
             }
         }
 
@@ -365,23 +434,37 @@ constexpr size_t AMP_SMEM = 2 * TILE_PAIRS * sizeof(CellPair) + 2 * sizeof(uint6
 
 typedef void (*amp_kernel_t)(const AmpArgs);
 
-template <int MODE, int QT, int MINB>
+template <int MODE, int QT, int MINB, int NB>
 static amp_kernel_t pick_split(bool split)
 {
-    return split ? (amp_kernel_t)k_amp<MODE, QT, true, MINB> : (amp_kernel_t)k_amp<MODE, QT, false, MINB>;
+    return split ? (amp_kernel_t)k_amp<MODE, QT, true, MINB, NB> : (amp_kernel_t)k_amp<MODE, QT, false, MINB, NB>;
 }
 
-// variant: 1 list direct, 2 polar direct, 4 cartesian direct (fp32 accumulation), 8 exact (fp64)
-static amp_kernel_t pick_kernel(int variant, int qt, bool split)
+template <int MODE>
+static amp_kernel_t pick_rec(int nb, bool split)
+{
+    switch (nb) {
+    case 1: return pick_split<MODE, 8, 2, 1>(split);
+    case 3: return pick_split<MODE, 8, 2, 3>(split);
+    case 4: return pick_split<MODE, 8, 2, 4>(split);
+    default: return pick_split<MODE, 8, 2, 2>(split);
+    }
+}
+
+// variant: 1 list direct, 2 polar direct, 4 cartesian direct, 3 polar recurrence, 5 cartesian recurrence
+// (all with fp32 accumulation over a tile), 8 exact (fp64)
+static amp_kernel_t pick_kernel(int variant, int qt, int nb, bool split)
 {
     switch (variant) {
-    case 1: return pick_split<2, 4, 3>(split);
+    case 1: return pick_split<2, 4, 3, 0>(split);
     case 2:
-        if (qt == 4) return pick_split<0, 4, 3>(split);
-        return pick_split<0, 8, 2>(split);
+        if (qt == 4) return pick_split<0, 4, 3, 0>(split);
+        return pick_split<0, 8, 2, 0>(split);
     case 4:
-        if (qt == 4) return pick_split<1, 4, 3>(split);
-        return pick_split<1, 8, 2>(split);
+        if (qt == 4) return pick_split<1, 4, 3, 0>(split);
+        return pick_split<1, 8, 2, 0>(split);
+    case 3: return pick_rec<0>(nb, split);
+    case 5: return pick_rec<1>(nb, split);
     default: return split ? (amp_kernel_t)k_amp_f64<true> : (amp_kernel_t)k_amp_f64<false>;
     }
 }
@@ -390,14 +473,17 @@ static int64_t ceil_div(int64_t a, int64_t b) { return (a + b - 1) / b; }
 
 nms_status plan_amplitude(nms_ctx* c, bool split, AmpPlan* plan)
 {
-    // precision policy: small problems run the exact fp64 kernel
+    // precision policy: small problems run the exact fp64 kernel; otherwise the line
+    // recurrence where the thread lines are equally spaced, else the direct kernel
     int variant;
     const bool small = (double)c->W * (double)c->n_q <= 1073741824.0;
+    const bool line_ok = c->g_type != 2 && c->g_uniform && c->g_n0 >= 2;
+    if (c->opt_variant == 2 && !line_ok)
+        return fail(c, NMS_E_UNSUPPORTED, "the line-recurrence variant needs a polar or Cartesian detector with equally spaced u0");
     if (c->opt_variant == 3 || (c->opt_variant == 0 && small)) variant = 8;
     else if (c->g_type == 2) variant = 1;
+    else if (c->opt_variant == 2 || (c->opt_variant == 0 && line_ok)) variant = (c->g_type == 0) ? 3 : 5;
     else variant = (c->g_type == 0) ? 2 : 4;
-    if (c->opt_variant == 2)
-        return fail(c, NMS_E_UNSUPPORTED, "the line-recurrence variant is not available for this detector / sample");
 
     // units of work along the cell dimension: tiles, or whole objects in split mode
     const int64_t units = split ? c->K : c->n_tiles;
@@ -406,6 +492,7 @@ nms_status plan_amplitude(nms_ctx* c, bool split, AmpPlan* plan)
     int qt_opts[3]; int n_opts = 0;
     if (variant == 8) { qt_opts[n_opts++] = 1; }
     else if (variant == 1) { qt_opts[n_opts++] = 4; }
+    else if (variant == 3 || variant == 5) { qt_opts[n_opts++] = 8; }
     else { qt_opts[n_opts++] = 8; qt_opts[n_opts++] = 4; }
     int qt = qt_opts[n_opts - 1];
     if (c->opt_qt && variant != 8) {
@@ -420,7 +507,7 @@ nms_status plan_amplitude(nms_ctx* c, bool split, AmpPlan* plan)
         }
     }
     const size_t smem = variant == 8 ? 0 : AMP_SMEM;
-    amp_kernel_t kern = pick_kernel(variant, qt, split);
+    amp_kernel_t kern = pick_kernel(variant, qt, c->opt_bases, split);
     NMS_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)AMP_SMEM));
     int occ = 0;
     NMS_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, AMP_THREADS, smem));
@@ -486,12 +573,12 @@ nms_status launch_amplitude(nms_ctx* c, const AmpPlan& plan, const int32_t* kind
     a.chunk_begin = plan.split ? (const int32_t*)c->chunk_begin.p : nullptr;
     a.n_tiles = (int)c->n_tiles;
     a.type = c->g_type; a.n0 = c->g_n0; a.n1 = c->g_n1; a.n_q = c->n_q;
-    a.u0 = (const float*)c->u0.p; a.qc = (const double2*)c->qc.p; a.sc = (const double2*)c->sc.p;
+    a.u0 = (const float*)c->u0.p; a.dq = c->g_dq; a.qc = (const double2*)c->qc.p; a.sc = (const double2*)c->sc.p;
     a.part = (double*)c->part.p; a.ppart = (double*)c->ppart.p; a.form = (double*)c->formpart.p;
     a.kinds = kinds_dev; a.n_kinds = n_kinds;
     a.rp.Px = c->P[0]; a.rp.Py = c->P[1]; a.rp.Pz = c->P[2]; a.rp.sN = c->sN; a.rp.sM = c->sM; a.rp.invV = c->invV;
 
-    amp_kernel_t kern = pick_kernel(plan.variant, plan.qt, plan.split);
+    amp_kernel_t kern = pick_kernel(plan.variant, plan.qt, c->opt_bases, plan.split);
     NMS_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)AMP_SMEM));
     dim3 grid((unsigned)plan.n_qblocks, (unsigned)n_chunks);
     timer_begin(c, NMS_T_AMPLITUDE);

@@ -168,17 +168,21 @@ static nms_status set_grid(nms_ctx* c, const nms_qgrid* g)
     c->g_type = g->type; c->g_n0 = g->n0; c->g_n1 = g->n1; c->n_q = (int64_t)g->n0 * g->n1;
     c->h_u0.assign(g->u0, g->u0 + g->n0);
     c->h_u1.assign(g->u1, g->u1 + len1);
-    // equally spaced along the thread line (u0)?  (decides whether the recurrence kernel may be used)
-    bool uni = g->type != 2;
-    if (uni && g->n0 > 2) {
-        const double a0 = g->u0[0], d = ((double)g->u0[g->n0 - 1] - a0) / (double)(g->n0 - 1);
+    // equally spaced along the thread line (u0)?  (decides whether the recurrence kernels may be used: every
+    // abscissa must lie within one fp32 ulp of the largest one from the progression u0[0] + i d)
+    bool uni = g->type != 2 && g->n0 >= 2;
+    double dq = 0.0;
+    if (uni) {
+        const double a0 = g->u0[0];
+        dq = ((double)g->u0[g->n0 - 1] - a0) / (double)(g->n0 - 1);
         double amax = 0.0, dev = 0.0;
         for (int i = 0; i < g->n0; ++i) {
             amax = fmax(amax, fabs((double)g->u0[i]));
-            dev = fmax(dev, fabs((double)g->u0[i] - (a0 + d * i)));
+            dev = fmax(dev, fabs((double)g->u0[i] - (a0 + dq * i)));
         }
-        uni = dev <= 4e-7 * amax;
+        uni = dq != 0.0 && dev <= 1.2e-7 * amax;
     }
+    c->g_dq = dq;
     c->g_uniform = uni;
     if (nms_status st = ensure(c, c->u0, sizeof(float) * (size_t)g->n0)) return st;
     if (nms_status st = ensure(c, c->u1, sizeof(float) * (size_t)len1)) return st;
@@ -452,6 +456,7 @@ nms_status nms_set_option(nms_ctx* c, const char* key, int64_t value)
     if (!strcmp(key, "variant")) { if (value < 0 || value > 3) return fail(c, NMS_E_ARG, "variant must be 0, 1, 2 or 3"); c->opt_variant = (int)value; }
     else if (!strcmp(key, "timing")) { c->opt_timing = value != 0; for (Timer& t : c->timers) t.used = 0; }
     else if (!strcmp(key, "chunks")) { if (value < 0) return fail(c, NMS_E_ARG, "chunks must be >= 0"); c->opt_chunks = (int)value; }
+    else if (!strcmp(key, "bases")) { if (value < 0 || value > 4) return fail(c, NMS_E_ARG, "bases must be 0..4"); c->opt_bases = (int)value; }
     else if (!strcmp(key, "qt")) { if (value != 0 && value != 4 && value != 8 && value != 16) return fail(c, NMS_E_ARG, "qt must be 0, 4, 8 or 16"); c->opt_qt = (int)value; }
     else return fail(c, NMS_E_ARG, "unknown option '%s'", key);
     return NMS_OK;

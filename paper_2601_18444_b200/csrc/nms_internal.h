@@ -58,10 +58,11 @@ struct nms_ctx {
     char err[512] = {0};
 
     // options
-    int opt_variant = 0;   // 0 auto, 1 direct, 2 recurrence
+    int opt_variant = 0;   // 0 auto, 1 direct, 2 recurrence, 3 exact fp64
     int opt_timing = 0;
     int opt_chunks = 0;
     int opt_qt = 0;        // 0 auto, else 4/8/16
+    int opt_bases = 0;     // recurrence kernels: exactly evaluated points per 8 (0 auto = 2, else 1..4)
     int64_t launches = 0;
     int variant_used = 0, n_chunks_used = 0, blocks_per_sm_used = 0, qt_used = 0;
 
@@ -88,7 +89,8 @@ struct nms_ctx {
     bool grid_valid = false;
     int g_type = 0, g_n0 = 0, g_n1 = 0;
     int64_t n_q = 0;
-    bool g_uniform = false;            // abscissa along the thread line (u0) is equally spaced
+    bool g_uniform = false;            // abscissa along the thread line (u0) is equally spaced (within 1 ulp)
+    double g_dq = 0.0;                 // its spacing (u0[n0-1] - u0[0]) / (n0 - 1)
     std::vector<float> h_u0, h_u1;
     nms::DevBuf u0, u1, qc, sc;        // qc: double2[n_q] (q_y,q_z) rad/nm; sc: double2[n_q] (sin th, cos th)
 
@@ -125,7 +127,7 @@ nms_status launch_prep(nms_ctx* c);                       // a-1: raw sample -> 
 nms_status launch_qsetup(nms_ctx* c);                     // detector abscissae -> qc, sc
 // k_amplitude.cu
 struct AmpPlan {
-    int variant;       // 1 general direct, 2 line direct, 3 line recurrence
+    int variant;       // 1 list direct, 2 polar direct, 4 cartesian direct, 3 polar / 5 cartesian recurrence, 8 exact
     int qt;            // q points per thread
     int n_chunks;
     int n_qblocks;
