@@ -47,6 +47,7 @@ namespace nms {
 
 constexpr int AMP_THREADS = 128;
 constexpr int TILE_PAIRS = TILE / 2;
+constexpr int STAGE_PAIRS = TILE_PAIRS + 1;   // one slack record: the software-pipelined loop reads one record ahead
 
 typedef unsigned long long u64;
 
@@ -268,14 +269,45 @@ __device__ __forceinline__ void rotate2(u64 c, u64 s, u64 cd, u64 sd, u64 nsd, u
     so = ffma2(c, sd, fmul2(s, cd));
 }
 
+// Segment b of the NB segments of a thread's QT points: [lo, hi], exactly evaluated at kb.
+template <int QT, int NB> struct Seg {
+    static __device__ __forceinline__ constexpr int lo(int b) { return (b * QT) / NB; }
+    static __device__ __forceinline__ constexpr int hi(int b) { return ((b + 1) * QT) / NB - 1; }
+    static __device__ __forceinline__ constexpr int kb(int b) { return lo(b) + (hi(b) - lo(b) + 1) / 2; }
+};
+
+// Recurrence kernels, everything one cell pair needs before its FP32 work: the weights, the step phasor
+// (phase step dq' p (polar) or dq' Z (Cartesian), exactly reduced) and the NB base phasors.
+template <int MODE, int NB>
+__device__ __forceinline__ void pair_phasors(const CellPair* __restrict__ rec, double c0, double c1, double dq,
+                                             const double (&gb)[NB], ulonglong2& w01, ulonglong2& w23, u64& cd, u64& sd,
+                                             u64 (&cb)[NB], u64 (&sb)[NB])
+{
+    const double2 Y = *reinterpret_cast<const double2*>(&rec->Ya);
+    const double2 Z = *reinterpret_cast<const double2*>(&rec->Za);
+    w01 = *reinterpret_cast<const ulonglong2*>(&rec->wN);
+    w23 = *reinterpret_cast<const ulonglong2*>(&rec->wy);
+    if (MODE == 0) {
+        const double pa = fma(c1, Z.x, c0 * Y.x), pb = fma(c1, Z.y, c0 * Y.y);   // Eq. 41 / q
+        phasor2(fma(dq, pa, MAGIC), fma(dq, pb, MAGIC), cd, sd);
+#pragma unroll
+        for (int b = 0; b < NB; ++b) phasor2(fma(gb[b], pa, MAGIC), fma(gb[b], pb, MAGIC), cb[b], sb[b]);
+    } else {
+        const double ua = c0 * Y.x, ub = c0 * Y.y;
+        phasor2(fma(dq, Z.x, MAGIC), fma(dq, Z.y, MAGIC), cd, sd);
+#pragma unroll
+        for (int b = 0; b < NB; ++b) phasor2(fma(gb[b], Z.x, ua) + MAGIC, fma(gb[b], Z.y, ub) + MAGIC, cb[b], sb[b]);
+    }
+}
+
 // NB = 0: direct evaluation of every pair; NB > 0: line recurrence with NB exactly evaluated points per QT
 template <int MODE, int QT, bool SPLIT, int MINB, int NB>
 __global__ void __launch_bounds__(AMP_THREADS, MINB) k_amp(const AmpArgs a)
 {
     static_assert(NB == 0 || (MODE != 2 && NB <= QT), "the recurrence needs a line of equally spaced abscissae");
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    CellPair* sC = reinterpret_cast<CellPair*>(smem_raw);                                  // [2][TILE_PAIRS]
-    uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + 2 * TILE_PAIRS * sizeof(CellPair));
+    CellPair* sC = reinterpret_cast<CellPair*>(smem_raw);                                  // [2][STAGE_PAIRS]
+    uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + 2 * STAGE_PAIRS * sizeof(CellPair));
 
     const int tid = threadIdx.x;
     const int chunk = blockIdx.y;
@@ -318,6 +350,9 @@ __global__ void __launch_bounds__(AMP_THREADS, MINB) k_amp(const AmpArgs a)
         for (int k = 1; k < QT; ++k)
             if (k >= kclamp) g[k] += (double)(k - (kclamp - 1)) * dq;   // g[k] was clamped to g[kclamp - 1]
     }
+    double gb[NB > 0 ? NB : 1];        // abscissae of the exactly evaluated points
+#pragma unroll
+    for (int b = 0; b < (NB > 0 ? NB : 1); ++b) gb[b] = g[Seg<QT, (NB > 0 ? NB : 1)>::kb(b)];
 
     if (tid == 0) {
         mbar_init(&bar[0], 1);
@@ -327,7 +362,7 @@ __global__ void __launch_bounds__(AMP_THREADS, MINB) k_amp(const AmpArgs a)
     __syncthreads();
     if (tid == 0) {
         if (tile_beg < tile_end) issue_tile(a, tile_beg, sC, &bar[0]);
-        if (tile_beg + 1 < tile_end) issue_tile(a, tile_beg + 1, sC + TILE_PAIRS, &bar[1]);
+        if (tile_beg + 1 < tile_end) issue_tile(a, tile_beg + 1, sC + STAGE_PAIRS, &bar[1]);
     }
 
     u64 acc[QT][8];
@@ -337,7 +372,7 @@ __global__ void __launch_bounds__(AMP_THREADS, MINB) k_amp(const AmpArgs a)
         const int it = t - tile_beg;
         const int stage = it & 1;
         const TileMeta tm = a.tiles[t];
-        const CellPair* __restrict__ tC = sC + stage * TILE_PAIRS;
+        const CellPair* __restrict__ tC = sC + stage * STAGE_PAIRS;
 #pragma unroll
         for (int k = 0; k < QT; ++k)
 #pragma unroll
@@ -345,16 +380,16 @@ __global__ void __launch_bounds__(AMP_THREADS, MINB) k_amp(const AmpArgs a)
         mbar_wait(&bar[stage], (uint32_t)((it >> 1) & 1));
 
         const int np = tm.n_slots >> 1;
+        if (NB == 0) {
 #pragma unroll 1
-        for (int j = 0; j < np; ++j) {
-            const double2 Y = *reinterpret_cast<const double2*>(&tC[j].Ya);
-            const double2 Z = *reinterpret_cast<const double2*>(&tC[j].Za);
-            const ulonglong2 w01 = *reinterpret_cast<const ulonglong2*>(&tC[j].wN);
-            const ulonglong2 w23 = *reinterpret_cast<const ulonglong2*>(&tC[j].wy);
-            double pa = 0.0, pb = 0.0;
-            if (MODE == 0) { pa = fma(c1, Z.x, c0 * Y.x); pb = fma(c1, Z.y, c0 * Y.y); }   // Eq. 41 / q
-            if (MODE == 1) { pa = c0 * Y.x; pb = c0 * Y.y; }
-            if (NB == 0) {
+            for (int j = 0; j < np; ++j) {
+                const double2 Y = *reinterpret_cast<const double2*>(&tC[j].Ya);
+                const double2 Z = *reinterpret_cast<const double2*>(&tC[j].Za);
+                const ulonglong2 w01 = *reinterpret_cast<const ulonglong2*>(&tC[j].wN);
+                const ulonglong2 w23 = *reinterpret_cast<const ulonglong2*>(&tC[j].wy);
+                double pa = 0.0, pb = 0.0;
+                if (MODE == 0) { pa = fma(c1, Z.x, c0 * Y.x); pb = fma(c1, Z.y, c0 * Y.y); }   // Eq. 41 / q
+                if (MODE == 1) { pa = c0 * Y.x; pb = c0 * Y.y; }
                 u64 x2[QT];
 #pragma unroll
                 for (int k = 0; k < QT; ++k) {
@@ -372,38 +407,46 @@ __global__ void __launch_bounds__(AMP_THREADS, MINB) k_amp(const AmpArgs a)
                     const u64 s2 = pack2(__sinf(xa), __sinf(xb));
                     accumulate(acc[k], w01, w23, c2, s2);
                 }
-            } else {
-                // step phasor of this cell pair: phase step dq' p (polar) or dq' Z (Cartesian), exactly reduced
-                u64 cd, sd;
-                if (MODE == 0) phasor2(fma(dq, pa, MAGIC), fma(dq, pb, MAGIC), cd, sd);
-                else           phasor2(fma(dq, Z.x, MAGIC), fma(dq, Z.y, MAGIC), cd, sd);
+            }
+        } else {
+            // software pipeline: the loads, fp64 phases and MUFU evaluations of pair j + 1 are issued
+            // alongside the FP32 rotations and accumulations of pair j (one basic block).  The read one
+            // record past the last pair stays inside the stage (slack record) and its result is dropped.
+            constexpr int NBX = NB > 0 ? NB : 1;
+            typedef Seg<QT, NBX> S;
+            ulonglong2 w01, w23;
+            u64 cd, sd, cb[NBX], sb[NBX];
+            pair_phasors<MODE, NBX>(tC, c0, c1, dq, gb, w01, w23, cd, sd, cb, sb);
+#pragma unroll 1
+            for (int j = 0; j < np; ++j) {
+                ulonglong2 w01n, w23n;
+                u64 cdn, sdn, cbn[NBX], sbn[NBX];
+                pair_phasors<MODE, NBX>(tC + j + 1, c0, c1, dq, gb, w01n, w23n, cdn, sdn, cbn, sbn);
                 const u64 nsd = sd ^ 0x8000000080000000ull;
 #pragma unroll
-                for (int b = 0; b < NB; ++b) {
-                    const int lo = (b * QT) / NB, hi = ((b + 1) * QT) / NB - 1;   // segment [lo, hi]
-                    const int kb = lo + (hi - lo + 1) / 2;                         // its exactly evaluated point
-                    u64 cb, sb;
-                    if (MODE == 0) phasor2(fma(g[kb], pa, MAGIC), fma(g[kb], pb, MAGIC), cb, sb);
-                    else           phasor2(fma(g[kb], Z.x, pa) + MAGIC, fma(g[kb], Z.y, pb) + MAGIC, cb, sb);
-                    accumulate(acc[kb], w01, w23, cb, sb);
-                    u64 c = cb, s = sb;
+                for (int b = 0; b < NBX; ++b) {
+                    accumulate(acc[S::kb(b)], w01, w23, cb[b], sb[b]);
+                    u64 c = cb[b], s = sb[b];
 #pragma unroll
-                    for (int k = kb + 1; k <= hi; ++k) {
+                    for (int k = S::kb(b) + 1; k <= S::hi(b); ++k) {
                         rotate2(c, s, cd, sd, nsd, c, s);
                         accumulate(acc[k], w01, w23, c, s);
                     }
-                    c = cb; s = sb;
+                    c = cb[b]; s = sb[b];
 #pragma unroll
-                    for (int k = kb - 1; k >= lo; --k) {
+                    for (int k = S::kb(b) - 1; k >= S::lo(b); --k) {
                         rotate2(c, s, cd, nsd, sd, c, s);
                         accumulate(acc[k], w01, w23, c, s);
                     }
                 }
+                w01 = w01n; w23 = w23n; cd = cdn; sd = sdn;
+#pragma unroll
+                for (int b = 0; b < NBX; ++b) { cb[b] = cbn[b]; sb[b] = sbn[b]; }
             }
         }
 
         __syncthreads();   // every thread is done with this stage: refill it while the flush runs
-        if (tid == 0 && t + 2 < tile_end) issue_tile(a, t + 2, sC + stage * TILE_PAIRS, &bar[stage]);
+        if (tid == 0 && t + 2 < tile_end) issue_tile(a, t + 2, sC + stage * STAGE_PAIRS, &bar[stage]);
 
         // ---- flush: add the fp32 tile sums to the fp64 chunk partials -----------------------------
         const bool first = (t == tile_beg);
@@ -430,7 +473,7 @@ __global__ void __launch_bounds__(AMP_THREADS, MINB) k_amp(const AmpArgs a)
 }
 
 // ---- host side: planning and dispatch ------------------------------------------------------------
-constexpr size_t AMP_SMEM = 2 * TILE_PAIRS * sizeof(CellPair) + 2 * sizeof(uint64_t);
+constexpr size_t AMP_SMEM = 2 * STAGE_PAIRS * sizeof(CellPair) + 2 * sizeof(uint64_t);
 
 typedef void (*amp_kernel_t)(const AmpArgs);
 

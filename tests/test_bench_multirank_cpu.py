@@ -1,0 +1,56 @@
+"""world_size-2 gloo test (CPU) of bench.py's multi-rank host logic (replicas only):
+the max-over-ranks reduction of the step time, the whole-job rate, and the reference arm's rank rule."""
+import json
+import os
+import subprocess
+import sys
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+WORKER = r"""
+import os, sys, json
+sys.path.insert(0, {root!r})
+import torch, torch.distributed as dist
+import bench
+dist.init_process_group(backend="gloo")
+rank, world = dist.get_rank(), dist.get_world_size()
+ms = bench.max_over_ranks(10.0 * (rank + 1), dist)          # ranks report 10 ms and 20 ms
+rate = bench.aggregate_rate(1_000_000_000, world, ms)       # 1e9 pairs per rank
+dist.barrier()
+if rank == 0:
+    print(json.dumps({{"ms": ms, "rate": rate, "world": world}}))
+dist.destroy_process_group()
+"""
+
+
+def test_max_over_ranks_and_aggregate_rate_gloo(tmp_path):
+    script = tmp_path / "worker.py"
+    script.write_text(WORKER.format(root=ROOT))
+    env = dict(os.environ, MASTER_ADDR="127.0.0.1")
+    out = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2",
+                          "--master-addr", "127.0.0.1", "--master-port", "29533", str(script)],
+                         capture_output=True, text=True, timeout=300, env=env, cwd=ROOT)
+    assert out.returncode == 0, out.stderr[-2000:]
+    line = [l for l in out.stdout.splitlines() if l.startswith("{")][-1]
+    d = json.loads(line)
+    assert d["world"] == 2
+    assert d["ms"] == pytest.approx(20.0)                      # the slower rank decides
+    assert d["rate"] == pytest.approx(2 * 1e9 / 20e-3 / 1e9)   # both ranks' pairs over the max time
+
+
+def test_single_process_helpers():
+    sys.path.insert(0, ROOT)
+    import bench
+    assert bench.max_over_ranks(3.5) == 3.5
+    assert bench.aggregate_rate(4_000_000_000, 1, 2000.0) == pytest.approx(2.0)
+
+
+def test_reference_arm_other_ranks_exit_without_work():
+    """Under torchrun only rank 0 runs the oracle arm; the other ranks exit 0 and print nothing."""
+    env = dict(os.environ, RANK="1", LOCAL_RANK="1", WORLD_SIZE="2")
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2"],
+                         capture_output=True, text=True, timeout=120, env=env, cwd=ROOT)
+    assert out.returncode == 0, out.stderr[-2000:]
+    assert out.stdout.strip() == ""

@@ -135,23 +135,27 @@ def _run_full(nms, h, wl, kinds):
 # C1, C2 at full size, full maps; every kernel variant the grid admits
 # ---------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("name", ["C1", "C2"])
-@pytest.mark.parametrize("variant,qt", [(0, 0), (3, 0), (1, 0), (1, 4), (1, 8)])
-def test_full_config_maps(nms, ctx, oracle_mod, name, variant, qt):
+@pytest.mark.parametrize("variant,qt,bases", [(0, 0, 0), (3, 0, 0), (1, 0, 0), (1, 4, 0), (1, 8, 0),
+                                               (2, 0, 0), (2, 0, 1), (2, 0, 2), (2, 0, 3), (2, 0, 4)])
+def test_full_config_maps(nms, ctx, oracle_mod, name, variant, qt, bases):
     """variant 0 = automatic (these small problems run the exact fp64 kernel: strict north_star criteria),
-    3 = exact forced, 1 = the fp32-accumulating direct kernels (reading 16 floor for NM and CHI)."""
+    3 = exact forced, 1 = the fp32-accumulating direct kernels, 2 = the line-recurrence kernels with
+    `bases` exactly evaluated points per 8 (reading 16 floor for NM and CHI in the fp32 kernels)."""
     wl = ni.make_config(name)
     kinds = list(ni.ALL_KINDS)
     _upload(nms, ctx, wl)
     nms.nms_set_option(ctx, "variant", variant)
     nms.nms_set_option(ctx, "qt", qt)
+    nms.nms_set_option(ctx, "bases", bases)
     A_gpu, M_gpu = _run_full(nms, ctx, wl, kinds)
     qy, qz, th = oracle_mod.grid_points(wl.grid)
     A, wsum, M = _oracle_maps(oracle_mod, wl, qy, qz, th, kinds)
     np.testing.assert_allclose(nms.nms_get_weight_sums(ctx), wsum, rtol=1e-12)
     assert_amplitudes(A_gpu, A, wsum, name)
-    assert_cross_sections(M_gpu, M, kinds, name, fp32=(variant == 1))
+    assert_cross_sections(M_gpu, M, kinds, name, fp32=(variant in (1, 2)))
     used = nms.nms_get_info(ctx, "variant_used")
-    assert used == (8 if variant != 1 else (2 if wl.grid.type == 0 else 4))
+    polar = wl.grid.type == 0
+    assert used == {0: 8, 3: 8, 1: 2 if polar else 4, 2: 3 if polar else 5}[variant]
 
 
 def test_c1_physics_on_gpu(nms, ctx):
@@ -172,8 +176,10 @@ def test_c1_physics_on_gpu(nms, ctx):
 # reduced C3, C4, C5 (same structure, several tiles and a ragged tail), full maps
 # ---------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("name", ["C3", "C4", "C5"])
-@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("variant", [0, 1, 2])
 def test_small_config_maps(nms, ctx, oracle_mod, name, variant):
+    if name == "C3" and variant == 2:
+        pytest.skip("C3's |q| is log-spaced: no line recurrence (NMS_E_UNSUPPORTED, see test_error_codes)")
     wl = ni.make_config(name, small=True)
     kinds = list(ni.ALL_KINDS)
     nms.nms_set_option(ctx, "variant", variant)
@@ -185,7 +191,40 @@ def test_small_config_maps(nms, ctx, oracle_mod, name, variant):
         A_gpu, M_gpu = _run_full(nms, ctx, wl, kinds)
         A, wsum, M = _oracle_maps(oracle_mod, wl, qy, qz, th, kinds, R=R)
         assert_amplitudes(A_gpu, A, wsum, name)
-        assert_cross_sections(M_gpu, M, kinds, name, fp32=(variant == 1))
+        assert_cross_sections(M_gpu, M, kinds, name, fp32=(variant in (1, 2)))
+
+
+@pytest.mark.parametrize("gtype", [0, 1])
+@pytest.mark.parametrize("n0", [1, 2, 7, 13, 24])
+def test_recurrence_ragged_lines(nms, ctx, oracle_mod, gtype, n0):
+    """Line recurrence on detector lines whose length is not a multiple of the 8 points a thread owns (and
+    shorter than them): the points beyond the edge continue the progression and are never stored."""
+    rng = np.random.Generator(np.random.Philox(4242))
+    W = 3000
+    pos = rng.uniform(-40, 40, size=(W, 3)).astype(np.float32)
+    N = rng.uniform(0.5, 1.5, size=W).astype(np.float32)
+    m = rng.normal(size=(W, 3)).astype(np.float32)
+    R = ni.rot_z(20.0) @ ni.rot_y(35.0) @ ni.rot_z(10.0)
+    if gtype == 0:
+        grid = ni.polar_grid(np.linspace(0.02, 1.7, n0) if n0 > 1 else np.array([0.5]), 37)
+    else:
+        grid = ni.cartesian_grid(np.linspace(-0.9, 1.1, n0) if n0 > 1 else np.array([0.3]), np.linspace(-1.0, 1.0, 37))
+    kinds = list(ni.ALL_KINDS)
+    import torch
+    nms.nms_set_sample(ctx, _t(pos), _t(N), _t(m), R)
+    nms.nms_set_option(ctx, "variant", 2 if n0 > 1 else 1)
+    amp = torch.empty((8, grid.n_q), dtype=torch.float32, device="cuda")
+    maps = torch.empty((len(kinds), grid.n_q), dtype=torch.float32, device="cuda")
+    nms.nms_amplitudes(ctx, grid, amp)
+    nms.nms_response(ctx, kinds, maps)
+    nms.nms_synchronize(ctx)
+    if n0 > 1:
+        assert nms.nms_get_info(ctx, "variant_used") == (3 if gtype == 0 else 5)
+    qy, qz, th = oracle_mod.grid_points(grid)
+    A, wsum = oracle_mod.amplitudes(pos, N, m, R, qy, qz, return_wsum=True)
+    M = oracle_mod.response(A, th, kinds)
+    assert_amplitudes(amp.cpu().numpy(), A, wsum, f"ragged n0={n0}")
+    assert_cross_sections(maps.cpu().numpy(), M, kinds, f"ragged n0={n0}", fp32=True)
 
 
 # ---------------------------------------------------------------------------------------------------
@@ -210,7 +249,8 @@ def test_full_size_sampled(nms, ctx, oracle_mod, name, n_sample):
         nms.nms_amplitudes(ctx, wl.grid, amp)
         nms.nms_response(ctx, kinds, maps)
         nms.nms_synchronize(ctx)
-        assert nms.nms_get_info(ctx, "variant_used") in (2, 3, 4)          # an fp32-accumulating kernel
+        # an fp32-accumulating kernel: direct for C3 (log-spaced |q|), line recurrence for C4 and C5
+        assert nms.nms_get_info(ctx, "variant_used") == {"C3": 2, "C4": 5, "C5": 3}[name]
         A_gpu, M_gpu = amp.cpu().numpy(), maps.cpu().numpy()
         A, wsum = oracle_mod.amplitudes(wl.pos, wl.N, wl.m, R, qy[idx], qz[idx], offsets=wl.offsets,
                                         centres=wl.centres, return_wsum=True)
