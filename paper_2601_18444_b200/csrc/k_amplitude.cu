@@ -4,9 +4,9 @@
 //
 // Work decomposition: grid = (detector blocks) x (cell chunks).  A block owns 128*QT detector points
 // (thread = one position along the fast detector index i1 and QT consecutive positions along i0) and
-// walks the tiles of its chunk.  Tiles (<= 512 cells as 256 CellPair records of 64 B) are brought into
-// shared memory by one elected thread with cp.async.bulk + mbarrier, double buffered; every lane of a warp
-// reads the same record (LDS.128 broadcast, no bank conflicts).
+// walks the tiles of its chunk.  Tiles (<= 512 Cell records of 32 B) are brought into shared memory by
+// one elected thread with cp.async.bulk + mbarrier, double buffered; every lane of a warp reads the same
+// record (2 LDS.128 broadcasts per cell, no bank conflicts).
 //
 // Arithmetic per (cell, detector point) -- B200 has three independent pipes that all get work:
 //   FP64 pipe : the phase in CYCLES, t = (q/2pi).r, by DFMA with the addend 1.5*2^20: the sum is rounded
@@ -15,12 +15,17 @@
 //               "t - rint(t)" reduction of the north star, done by the rounding of the adder, with no fp32
 //               phase rounding and no tile origins;
 //   conversion: one I2FP turns that word into a float (|error| <= 2^-25 cycle = 1.9e-7 rad);
-//   FP32 pipe : packed mul/fma.rn.f32x2 over the two cells of a CellPair: x = 2 pi frac (1 op), then the
-//               8 accumulations w_c cos, w_c sin (4 packed ops per pair);
-//   XU pipe   : sin.approx / cos.approx of x in [-pi, pi) (absolute error 2^-21.4, CUDA C Programming Guide).
-// Accumulators are fp32 over one tile only (<= 256 additions per packed half); at the end of a tile they
-// are added to fp64 chunk partials in global memory (block-private slots, plain read-modify-write,
-// deterministic).  The epilogue kernel sums the chunks and forms the responses.
+//   XU pipe   : sin.approx / cos.approx of x = 2 pi frac in [-pi, pi) (absolute error 2^-21.4, CUDA C
+//               Programming Guide), written into an aligned register pair {cos, sin};
+//   FP32 pipe : 4 packed fma.rn.f32x2 per pair, one per weight channel: {w, w} * {cos, sin} + {Re, -Im},
+//               the weight as a 32-bit broadcast operand (an FFMA2 with three 64-bit register operands
+//               was measured at 3 cycles instead of 2: register-file bandwidth).
+//               A complex accumulator is ONE 64-bit register pair, so a detector point costs 8 registers
+//               and a thread with QT = 8 points needs 64 accumulator registers: 4 blocks of 128 threads
+//               per SM (16 warps) instead of 2, which is what hides the MUFU / FP64 / LDS latencies.
+// Accumulators are fp32 over one tile only (<= 512 additions); at the end of a tile they are added to
+// fp64 chunk partials in global memory (block-private slots, plain read-modify-write, deterministic).
+// The epilogue kernel sums the chunks and forms the responses.
 //
 // Phase variants (MODE): how t is formed for the thread's QT points
 //   0  polar   : p = sin(th) Y + cos(th) Z per (cell, thread) [2 fp64 ops], t_k = q'_k p + magic [1 per pair]
@@ -35,19 +40,18 @@
 // point per segment (its "base") is evaluated exactly as above -- the resync, at EVERY cell -- and the
 // others are reached from it by at most ceil((QT/NB - 1)/2) complex rotations with the step phasor
 // (cos, sin of the exactly reduced step phase, one evaluation per cell and thread), forwards or backwards
-// (conjugate step).  A rotation is 2 packed multiplies + 2 packed FMAs per cell pair, so a pair costs
-// 12 FP32 lane-operations and the MUFU load drops from 2 to (NB + 1) * 2 / QT per pair.  Error: a point
-// s steps from its base carries (s + 1) MUFU errors (2^-21.4 each) and s fp32 roundings, and the deviation
-// of the fp32 abscissae from the exact progression (<= 1 ulp of q, checked on the host) enters as a phase
-// error <= ulp(q) * |r|; both are measured against the oracle in tests/test_gpu_parity.py.
+// (conjugate step).  A rotation is 2 FMUL + 2 FFMA, so a pair costs 12 FP32 lane-operations and the MUFU
+// load drops from 2 to (NB + 1) * 2 / QT per pair.  Error: a point s steps from its base carries (s + 1)
+// MUFU errors (2^-21.4 each) and s fp32 roundings, and the deviation of the fp32 abscissae from the exact
+// progression (<= 1 ulp of q, checked on the host) enters as a phase error <= ulp(q) * |r|; both are
+// measured against the oracle in tests/test_gpu_parity.py.
 #include "nms_internal.h"
 #include "nms_response.cuh"
 
 namespace nms {
 
 constexpr int AMP_THREADS = 128;
-constexpr int TILE_PAIRS = TILE / 2;
-constexpr int STAGE_PAIRS = TILE_PAIRS + 1;   // one slack record: the software-pipelined loop reads one record ahead
+constexpr int STAGE_CELLS = TILE;
 
 typedef unsigned long long u64;
 
@@ -55,7 +59,7 @@ constexpr double MAGIC = 1572864.0;                 // 1.5 * 2^20: ulp = 2^-32 (
 constexpr double INV_2PI = 0.15915494309189533577;
 
 struct AmpArgs {
-    const CellPair* cells;
+    const Cell* cells;
     const TileMeta* tiles;
     const int32_t* chunk_begin;   // [n_chunks+1] or NULL (equal parts of n_tiles)
     int n_tiles;
@@ -101,13 +105,13 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
                      smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
-__device__ __forceinline__ void issue_tile(const AmpArgs& a, int tile, CellPair* dst, uint64_t* bar)
+__device__ __forceinline__ void issue_tile(const AmpArgs& a, int tile, Cell* dst, uint64_t* bar)
 {
     const TileMeta tm = a.tiles[tile];
-    const uint32_t bytes = (uint32_t)(tm.n_slots / 2) * (uint32_t)sizeof(CellPair);
+    const uint32_t bytes = (uint32_t)tm.n_slots * (uint32_t)sizeof(Cell);
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     mbar_expect_tx(bar, bytes);
-    bulk_g2s(dst, a.cells + tm.first_slot / 2, bytes, bar);
+    bulk_g2s(dst, a.cells + tm.first_slot, bytes, bar);
 }
 
 // ---- packed fp32x2 arithmetic (sm_100 PTX; SASS FFMA2) -------------------------------------------
@@ -134,24 +138,44 @@ __device__ __forceinline__ u64 fmul2(u64 a, u64 b)
     return d;
 }
 
-// The low words of ma, mb hold frac(t) * 2^32 as signed integers (t = phase in cycles, see MAGIC) ->
-// x = 2 pi frac in [-pi, pi), packed.  One I2FP each (24 significant bits: |error| <= 2^-25 cycle) and
-// one packed multiply.
-__device__ __forceinline__ u64 phase_to_x(double ma, double mb)
+// The low word of m holds frac(t) * 2^32 as a signed integer (t = phase in cycles, see MAGIC).  One I2FP
+// (24 significant bits: |error| <= 2^-25 cycle) and one multiply give x = 2 pi frac in [-pi, pi); the
+// phasor {cos x, sin x} comes back as one packed register pair.
+__device__ __forceinline__ u64 phasor(double m)
 {
     const float TWO_PI_2M32 = 0x1.921fb6p-30f;   // fl(2 pi) * 2^-32
-    const float fa = __int2float_rn(__double2loint(ma));
-    const float fb = __int2float_rn(__double2loint(mb));
-    return fmul2(pack2(fa, fb), pack2(TWO_PI_2M32, TWO_PI_2M32));
+#if defined(ABL) && (ABL == 1)
+    const float x = __int2float_rn(__double2loint(m)) * TWO_PI_2M32;
+    return pack2(x, x * 0.5f);
+#elif defined(ABL) && (ABL == 2)
+    const float x = __int_as_float(__double2loint(m)) * TWO_PI_2M32;
+    return pack2(x, x * 0.5f);
+#elif defined(ABL) && (ABL == 4)
+    const float x = __int2float_rn(__double2loint(m)) * TWO_PI_2M32;
+    return pack2(exp2f(x), exp2f(x + 1.0f));
+#else
+    const float x = __int2float_rn(__double2loint(m)) * TWO_PI_2M32;
+    return pack2(__cosf(x), __sinf(x));
+#endif
 }
 
-// 8 accumulations of one (cell pair, detector point): acc[2c] += w_c cos, acc[2c+1] += w_c sin, packed {a, b}
-__device__ __forceinline__ void accumulate(u64 (&acc)[8], const ulonglong2& w01, const ulonglong2& w23, u64 c2, u64 s2)
+// 4 packed accumulations of one (cell, detector point): acc[c] += {w_c, w_c} * {cos, sin}.  The pack of a
+// register with itself compiles to the broadcast operand form (FFMA2 Rd, Rw.F32, Rph, Racc): no extra move.
+__device__ __forceinline__ void accumulate(u64 (&acc)[4], const float4& w, u64 ph)
 {
-    acc[0] = ffma2(w01.x, c2, acc[0]); acc[1] = ffma2(w01.x, s2, acc[1]);
-    acc[2] = ffma2(w01.y, c2, acc[2]); acc[3] = ffma2(w01.y, s2, acc[3]);
-    acc[4] = ffma2(w23.x, c2, acc[4]); acc[5] = ffma2(w23.x, s2, acc[5]);
-    acc[6] = ffma2(w23.y, c2, acc[6]); acc[7] = ffma2(w23.y, s2, acc[7]);
+    acc[0] = ffma2(pack2(w.x, w.x), ph, acc[0]);
+    acc[1] = ffma2(pack2(w.y, w.y), ph, acc[1]);
+    acc[2] = ffma2(pack2(w.z, w.z), ph, acc[2]);
+    acc[3] = ffma2(pack2(w.w, w.w), ph, acc[3]);
+}
+
+// Advance the phase of the phasor {c, s} by the step whose phasor is (cd, sd): {c cd - s sd, s cd + c sd}.
+// The backward rotation passes (cd, -sd).  2 FMUL + 2 FFMA.
+__device__ __forceinline__ u64 rotate(u64 ph, float cd, float sd)
+{
+    float c, s;
+    unpack2(ph, c, s);
+    return pack2(fmaf(c, cd, -(s * sd)), fmaf(c, sd, s * cd));
 }
 
 // Add the sums Ap[8] of one tile at detector point f to the fp64 chunk partials (block-private slots, plain
@@ -222,27 +246,21 @@ __global__ void __launch_bounds__(AMP_THREADS) k_amp_f64(const AmpArgs a)
     bool first_total = true;
     for (int t = tile_beg; t < tile_end; ++t) {
         const TileMeta tm = a.tiles[t];
-        const CellPair* __restrict__ tC = a.cells + tm.first_slot / 2;
+        const Cell* __restrict__ tC = a.cells + tm.first_slot;
         double Ap[8];
 #pragma unroll
         for (int r = 0; r < 8; ++r) Ap[r] = 0.0;
-        const int np = tm.n_slots >> 1;
-        for (int j = 0; j < np; ++j) {
-            const CellPair cp = tC[j];
+        for (int j = 0; j < tm.n_slots; ++j) {
+            const Cell ce = tC[j];
+            double ph = fma(qz, ce.Z, qy * ce.Y);          // Eq. 41, in cycles
+            ph -= rint(ph);
+            double sn, cs;
+            sincospi(2.0 * ph, &sn, &cs);
+            const double w[4] = {(double)ce.wN, (double)ce.wx, (double)ce.wy, (double)ce.wz};
 #pragma unroll
-            for (int half = 0; half < 2; ++half) {
-                const double Y = half ? cp.Yb : cp.Ya, Z = half ? cp.Zb : cp.Za;
-                double ph = fma(qz, Z, qy * Y);          // Eq. 41, in cycles
-                ph -= rint(ph);
-                double sn, cs;
-                sincospi(2.0 * ph, &sn, &cs);
-                const double w[4] = {(double)(half ? cp.wN.y : cp.wN.x), (double)(half ? cp.wx.y : cp.wx.x),
-                                     (double)(half ? cp.wy.y : cp.wy.x), (double)(half ? cp.wz.y : cp.wz.x)};
-#pragma unroll
-                for (int c = 0; c < 4; ++c) {
-                    Ap[2 * c] = fma(w[c], cs, Ap[2 * c]);            // Re: + sum w cos(Psi)   (Eq. 44, 46)
-                    Ap[2 * c + 1] = fma(-w[c], sn, Ap[2 * c + 1]);   // Im: - sum w sin(Psi)   (Eq. 45, 47)
-                }
+            for (int c = 0; c < 4; ++c) {
+                Ap[2 * c] = fma(w[c], cs, Ap[2 * c]);            // Re: + sum w cos(Psi)   (Eq. 44, 46)
+                Ap[2 * c + 1] = fma(-w[c], sn, Ap[2 * c + 1]);   // Im: - sum w sin(Psi)   (Eq. 45, 47)
             }
         }
         const bool p_first = SPLIT ? ((tm.flags & 2) != 0) : false;
@@ -252,23 +270,6 @@ __global__ void __launch_bounds__(AMP_THREADS) k_amp_f64(const AmpArgs a)
     }
 }
 
-// phasor of the exactly reduced phases (ma, mb) of the two cells of a pair: packed cos and sin
-__device__ __forceinline__ void phasor2(double ma, double mb, u64& c2, u64& s2)
-{
-    float xa, xb;
-    unpack2(phase_to_x(ma, mb), xa, xb);
-    c2 = pack2(__cosf(xa), __cosf(xb));
-    s2 = pack2(__sinf(xa), __sinf(xb));
-}
-
-// (c, s) -> (c cd - s sd, s cd + c sd): advance the phase by the step whose phasor is (cd, sd); nsd = -sd.
-// The backward rotation passes (cd, nsd, sd).
-__device__ __forceinline__ void rotate2(u64 c, u64 s, u64 cd, u64 sd, u64 nsd, u64& co, u64& so)
-{
-    co = ffma2(c, cd, fmul2(s, nsd));
-    so = ffma2(c, sd, fmul2(s, cd));
-}
-
 // Segment b of the NB segments of a thread's QT points: [lo, hi], exactly evaluated at kb.
 template <int QT, int NB> struct Seg {
     static __device__ __forceinline__ constexpr int lo(int b) { return (b * QT) / NB; }
@@ -276,38 +277,14 @@ template <int QT, int NB> struct Seg {
     static __device__ __forceinline__ constexpr int kb(int b) { return lo(b) + (hi(b) - lo(b) + 1) / 2; }
 };
 
-// Recurrence kernels, everything one cell pair needs before its FP32 work: the weights, the step phasor
-// (phase step dq' p (polar) or dq' Z (Cartesian), exactly reduced) and the NB base phasors.
-template <int MODE, int NB>
-__device__ __forceinline__ void pair_phasors(const CellPair* __restrict__ rec, double c0, double c1, double dq,
-                                             const double (&gb)[NB], ulonglong2& w01, ulonglong2& w23, u64& cd, u64& sd,
-                                             u64 (&cb)[NB], u64 (&sb)[NB])
-{
-    const double2 Y = *reinterpret_cast<const double2*>(&rec->Ya);
-    const double2 Z = *reinterpret_cast<const double2*>(&rec->Za);
-    w01 = *reinterpret_cast<const ulonglong2*>(&rec->wN);
-    w23 = *reinterpret_cast<const ulonglong2*>(&rec->wy);
-    if (MODE == 0) {
-        const double pa = fma(c1, Z.x, c0 * Y.x), pb = fma(c1, Z.y, c0 * Y.y);   // Eq. 41 / q
-        phasor2(fma(dq, pa, MAGIC), fma(dq, pb, MAGIC), cd, sd);
-#pragma unroll
-        for (int b = 0; b < NB; ++b) phasor2(fma(gb[b], pa, MAGIC), fma(gb[b], pb, MAGIC), cb[b], sb[b]);
-    } else {
-        const double ua = c0 * Y.x, ub = c0 * Y.y;
-        phasor2(fma(dq, Z.x, MAGIC), fma(dq, Z.y, MAGIC), cd, sd);
-#pragma unroll
-        for (int b = 0; b < NB; ++b) phasor2(fma(gb[b], Z.x, ua) + MAGIC, fma(gb[b], Z.y, ub) + MAGIC, cb[b], sb[b]);
-    }
-}
-
 // NB = 0: direct evaluation of every pair; NB > 0: line recurrence with NB exactly evaluated points per QT
 template <int MODE, int QT, bool SPLIT, int MINB, int NB>
 __global__ void __launch_bounds__(AMP_THREADS, MINB) k_amp(const AmpArgs a)
 {
     static_assert(NB == 0 || (MODE != 2 && NB <= QT), "the recurrence needs a line of equally spaced abscissae");
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    CellPair* sC = reinterpret_cast<CellPair*>(smem_raw);                                  // [2][STAGE_PAIRS]
-    uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + 2 * STAGE_PAIRS * sizeof(CellPair));
+    Cell* sC = reinterpret_cast<Cell*>(smem_raw);                                          // [2][STAGE_CELLS]
+    uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + 2 * STAGE_CELLS * sizeof(Cell));
 
     const int tid = threadIdx.x;
     const int chunk = blockIdx.y;
@@ -345,14 +322,16 @@ __global__ void __launch_bounds__(AMP_THREADS, MINB) k_amp(const AmpArgs a)
     if (MODE == 1) c0 = h[0];
     (void)c1;
     const double dq = a.dq * INV_2PI;   // recurrence: spacing of the line in cycles/nm
+    constexpr int NBX = NB > 0 ? NB : 1;
+    typedef Seg<QT, NBX> S;
+    double gb[NBX];                     // abscissae of the exactly evaluated points
     if (NB > 0) {                       // points beyond the detector edge continue the progression (never stored)
 #pragma unroll
         for (int k = 1; k < QT; ++k)
             if (k >= kclamp) g[k] += (double)(k - (kclamp - 1)) * dq;   // g[k] was clamped to g[kclamp - 1]
     }
-    double gb[NB > 0 ? NB : 1];        // abscissae of the exactly evaluated points
 #pragma unroll
-    for (int b = 0; b < (NB > 0 ? NB : 1); ++b) gb[b] = g[Seg<QT, (NB > 0 ? NB : 1)>::kb(b)];
+    for (int b = 0; b < NBX; ++b) gb[b] = g[S::kb(b)];
 
     if (tid == 0) {
         mbar_init(&bar[0], 1);
@@ -362,91 +341,76 @@ __global__ void __launch_bounds__(AMP_THREADS, MINB) k_amp(const AmpArgs a)
     __syncthreads();
     if (tid == 0) {
         if (tile_beg < tile_end) issue_tile(a, tile_beg, sC, &bar[0]);
-        if (tile_beg + 1 < tile_end) issue_tile(a, tile_beg + 1, sC + STAGE_PAIRS, &bar[1]);
+        if (tile_beg + 1 < tile_end) issue_tile(a, tile_beg + 1, sC + STAGE_CELLS, &bar[1]);
     }
 
-    u64 acc[QT][8];
+    u64 acc[QT][4];            // per point and channel: {sum w cos, sum w sin}
     bool first_total = true;   // SPLIT: no object of this chunk has been completed yet
 
     for (int t = tile_beg; t < tile_end; ++t) {
         const int it = t - tile_beg;
         const int stage = it & 1;
         const TileMeta tm = a.tiles[t];
-        const CellPair* __restrict__ tC = sC + stage * STAGE_PAIRS;
+        const Cell* __restrict__ tC = sC + stage * STAGE_CELLS;
 #pragma unroll
         for (int k = 0; k < QT; ++k)
 #pragma unroll
-            for (int r = 0; r < 8; ++r) acc[k][r] = 0ull;
+            for (int r = 0; r < 4; ++r) acc[k][r] = 0ull;
         mbar_wait(&bar[stage], (uint32_t)((it >> 1) & 1));
 
-        const int np = tm.n_slots >> 1;
-        if (NB == 0) {
+        const int nc = tm.n_slots;
+#if defined(ABL) && (ABL == 3)
 #pragma unroll 1
-            for (int j = 0; j < np; ++j) {
-                const double2 Y = *reinterpret_cast<const double2*>(&tC[j].Ya);
-                const double2 Z = *reinterpret_cast<const double2*>(&tC[j].Za);
-                const ulonglong2 w01 = *reinterpret_cast<const ulonglong2*>(&tC[j].wN);
-                const ulonglong2 w23 = *reinterpret_cast<const ulonglong2*>(&tC[j].wy);
-                double pa = 0.0, pb = 0.0;
-                if (MODE == 0) { pa = fma(c1, Z.x, c0 * Y.x); pb = fma(c1, Z.y, c0 * Y.y); }   // Eq. 41 / q
-                if (MODE == 1) { pa = c0 * Y.x; pb = c0 * Y.y; }
-                u64 x2[QT];
+#else
+#pragma unroll 2
+#endif
+        for (int j = 0; j < nc; ++j) {
+            const double2 YZ = *reinterpret_cast<const double2*>(&tC[j].Y);
+            const float4 w = *reinterpret_cast<const float4*>(&tC[j].wN);
+            double p = 0.0;
+            if (MODE == 0) p = fma(c1, YZ.y, c0 * YZ.x);   // Eq. 41 / q
+            if (MODE == 1) p = c0 * YZ.x;
+            if (NB == 0) {
+                u64 ph[QT];
 #pragma unroll
                 for (int k = 0; k < QT; ++k) {
-                    double ma, mb;
-                    if (MODE == 0) { ma = fma(g[k], pa, MAGIC); mb = fma(g[k], pb, MAGIC); }
-                    else if (MODE == 1) { ma = fma(g[k], Z.x, pa) + MAGIC; mb = fma(g[k], Z.y, pb) + MAGIC; }
-                    else { ma = fma(g[k], Z.x, h[k] * Y.x) + MAGIC; mb = fma(g[k], Z.y, h[k] * Y.y) + MAGIC; }
-                    x2[k] = phase_to_x(ma, mb);
+                    double m;
+                    if (MODE == 0) m = fma(g[k], p, MAGIC);
+                    else if (MODE == 1) m = fma(g[k], YZ.y, p) + MAGIC;
+                    else m = fma(g[k], YZ.y, h[k] * YZ.x) + MAGIC;
+                    ph[k] = phasor(m);
                 }
 #pragma unroll
-                for (int k = 0; k < QT; ++k) {
-                    float xa, xb;
-                    unpack2(x2[k], xa, xb);
-                    const u64 c2 = pack2(__cosf(xa), __cosf(xb));
-                    const u64 s2 = pack2(__sinf(xa), __sinf(xb));
-                    accumulate(acc[k], w01, w23, c2, s2);
-                }
-            }
-        } else {
-            // software pipeline: the loads, fp64 phases and MUFU evaluations of pair j + 1 are issued
-            // alongside the FP32 rotations and accumulations of pair j (one basic block).  The read one
-            // record past the last pair stays inside the stage (slack record) and its result is dropped.
-            constexpr int NBX = NB > 0 ? NB : 1;
-            typedef Seg<QT, NBX> S;
-            ulonglong2 w01, w23;
-            u64 cd, sd, cb[NBX], sb[NBX];
-            pair_phasors<MODE, NBX>(tC, c0, c1, dq, gb, w01, w23, cd, sd, cb, sb);
-#pragma unroll 1
-            for (int j = 0; j < np; ++j) {
-                ulonglong2 w01n, w23n;
-                u64 cdn, sdn, cbn[NBX], sbn[NBX];
-                pair_phasors<MODE, NBX>(tC + j + 1, c0, c1, dq, gb, w01n, w23n, cdn, sdn, cbn, sbn);
-                const u64 nsd = sd ^ 0x8000000080000000ull;
+                for (int k = 0; k < QT; ++k) accumulate(acc[k], w, ph[k]);
+            } else {
+                // step phasor of this cell: phase step dq' p (polar) or dq' Z (Cartesian), exactly reduced
+                float cd, sd;
+                unpack2(phasor(fma(dq, MODE == 0 ? p : YZ.y, MAGIC)), cd, sd);
+                u64 pb[NBX];
+#pragma unroll
+                for (int b = 0; b < NBX; ++b)
+                    pb[b] = phasor(MODE == 0 ? fma(gb[b], p, MAGIC) : fma(gb[b], YZ.y, p) + MAGIC);
 #pragma unroll
                 for (int b = 0; b < NBX; ++b) {
-                    accumulate(acc[S::kb(b)], w01, w23, cb[b], sb[b]);
-                    u64 c = cb[b], s = sb[b];
+                    accumulate(acc[S::kb(b)], w, pb[b]);
+                    u64 ph = pb[b];
 #pragma unroll
                     for (int k = S::kb(b) + 1; k <= S::hi(b); ++k) {
-                        rotate2(c, s, cd, sd, nsd, c, s);
-                        accumulate(acc[k], w01, w23, c, s);
+                        ph = rotate(ph, cd, sd);
+                        accumulate(acc[k], w, ph);
                     }
-                    c = cb[b]; s = sb[b];
+                    ph = pb[b];
 #pragma unroll
                     for (int k = S::kb(b) - 1; k >= S::lo(b); --k) {
-                        rotate2(c, s, cd, nsd, sd, c, s);
-                        accumulate(acc[k], w01, w23, c, s);
+                        ph = rotate(ph, cd, -sd);
+                        accumulate(acc[k], w, ph);
                     }
                 }
-                w01 = w01n; w23 = w23n; cd = cdn; sd = sdn;
-#pragma unroll
-                for (int b = 0; b < NBX; ++b) { cb[b] = cbn[b]; sb[b] = sbn[b]; }
             }
         }
 
         __syncthreads();   // every thread is done with this stage: refill it while the flush runs
-        if (tid == 0 && t + 2 < tile_end) issue_tile(a, t + 2, sC + stage * STAGE_PAIRS, &bar[stage]);
+        if (tid == 0 && t + 2 < tile_end) issue_tile(a, t + 2, sC + stage * STAGE_CELLS, &bar[stage]);
 
         // ---- flush: add the fp32 tile sums to the fp64 chunk partials -----------------------------
         const bool first = (t == tile_beg);
@@ -459,11 +423,10 @@ __global__ void __launch_bounds__(AMP_THREADS, MINB) k_amp(const AmpArgs a)
                 double Ap[8];
 #pragma unroll
                 for (int w = 0; w < 4; ++w) {
-                    float ca, cb, sa, sb;
-                    unpack2(acc[k][2 * w], ca, cb);
-                    unpack2(acc[k][2 * w + 1], sa, sb);
-                    Ap[2 * w] = (double)ca + (double)cb;          // Re: + sum w cos(Psi)   (Eq. 44, 46)
-                    Ap[2 * w + 1] = -((double)sa + (double)sb);   // Im: - sum w sin(Psi)   (Eq. 45, 47)
+                    float cs, sn;
+                    unpack2(acc[k][w], cs, sn);
+                    Ap[2 * w] = (double)cs;          // Re: + sum w cos(Psi)   (Eq. 44, 46)
+                    Ap[2 * w + 1] = -(double)sn;     // Im: - sum w sin(Psi)   (Eq. 45, 47)
                 }
                 flush_point<SPLIT>(a, chunk, f, Ap, first, p_first, p_last, first_total);
             }
@@ -473,7 +436,7 @@ __global__ void __launch_bounds__(AMP_THREADS, MINB) k_amp(const AmpArgs a)
 }
 
 // ---- host side: planning and dispatch ------------------------------------------------------------
-constexpr size_t AMP_SMEM = 2 * STAGE_PAIRS * sizeof(CellPair) + 2 * sizeof(uint64_t);
+constexpr size_t AMP_SMEM = 2 * STAGE_CELLS * sizeof(Cell) + 2 * sizeof(uint64_t);
 
 typedef void (*amp_kernel_t)(const AmpArgs);
 
@@ -487,10 +450,10 @@ template <int MODE>
 static amp_kernel_t pick_rec(int nb, bool split)
 {
     switch (nb) {
-    case 1: return pick_split<MODE, 8, 2, 1>(split);
-    case 3: return pick_split<MODE, 8, 2, 3>(split);
-    case 4: return pick_split<MODE, 8, 2, 4>(split);
-    default: return pick_split<MODE, 8, 2, 2>(split);
+    case 1: return pick_split<MODE, 8, 4, 1>(split);
+    case 3: return pick_split<MODE, 8, 4, 3>(split);
+    case 4: return pick_split<MODE, 8, 4, 4>(split);
+    default: return pick_split<MODE, 8, 4, 2>(split);
     }
 }
 
@@ -499,13 +462,13 @@ static amp_kernel_t pick_rec(int nb, bool split)
 static amp_kernel_t pick_kernel(int variant, int qt, int nb, bool split)
 {
     switch (variant) {
-    case 1: return pick_split<2, 4, 3, 0>(split);
+    case 1: return pick_split<2, 4, 4, 0>(split);
     case 2:
-        if (qt == 4) return pick_split<0, 4, 3, 0>(split);
-        return pick_split<0, 8, 2, 0>(split);
+        if (qt == 4) return pick_split<0, 4, 4, 0>(split);
+        return pick_split<0, 8, 4, 0>(split);
     case 4:
-        if (qt == 4) return pick_split<1, 4, 3, 0>(split);
-        return pick_split<1, 8, 2, 0>(split);
+        if (qt == 4) return pick_split<1, 4, 4, 0>(split);
+        return pick_split<1, 8, 4, 0>(split);
     case 3: return pick_rec<0>(nb, split);
     case 5: return pick_rec<1>(nb, split);
     default: return split ? (amp_kernel_t)k_amp_f64<true> : (amp_kernel_t)k_amp_f64<false>;
@@ -611,7 +574,7 @@ nms_status launch_amplitude(nms_ctx* c, const AmpPlan& plan, const int32_t* kind
         if (nms_status st = ensure(c, c->formpart, sizeof(double) * (size_t)n_kinds * (size_t)c->n_q * n_chunks)) return st;
     }
     AmpArgs a;
-    a.cells = (const CellPair*)c->cells.p;
+    a.cells = (const Cell*)c->cells.p;
     a.tiles = (const TileMeta*)c->tile_meta.p;
     a.chunk_begin = plan.split ? (const int32_t*)c->chunk_begin.p : nullptr;
     a.n_tiles = (int)c->n_tiles;

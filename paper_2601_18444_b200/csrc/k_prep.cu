@@ -1,8 +1,8 @@
 // k_prep.cu -- a-1: rotate + pack the real-space sample into tiles, and detector set-up.
 //
 //  prep kernel   (Eq. 37-41):  r' = R (x + r^k), m' = R m in fp64; only Y, Z (rows 2, 3 of R)
-//                are kept because q_x = 0 on the detector (Eq. 41).  One block per tile, one thread per
-//                cell pair: it writes the CellPair record (fp64 Y, Z; weights rounded once to fp32), finds
+//                are kept because q_x = 0 on the detector (Eq. 41).  One block per tile, two cells per
+//                thread: it writes the Cell records (fp64 Y, Z; weights rounded once to fp32), finds
 //                the tile's bounding-box midpoint (Y0, Z0) and extent, and accumulates sum_j |w_cj| for
 //                the tolerance denominators.
 //  qsetup kernel (Eq. 6): per detector point (q_y, q_z) in fp64 [rad/nm] and
@@ -23,7 +23,7 @@ struct PrepArgs {
     const int64_t* first_slot;
     const int32_t* flags;
     TileMeta* meta;
-    CellPair* cells;
+    Cell* cells;
     double* wsum;
     double R[9];
 };
@@ -113,12 +113,15 @@ __global__ void __launch_bounds__(PREP_THREADS) k_prep(const PrepArgs a)
         for (int r = 0; r < 4; ++r)
             if (v[4 + r] != 0.0) atomicAdd(a.wsum + r, v[4 + r]);
     }
-    if (2 * tid < n_slots) {   // cells beyond n_src are the zero-weight padding (Y = Z = 0, w = 0)
-        CellPair cp;
-        cp.Ya = Y[0]; cp.Yb = Y[1]; cp.Za = Z[0]; cp.Zb = Z[1];
-        cp.wN = make_float2(wN[0], wN[1]); cp.wx = make_float2(wx[0], wx[1]);
-        cp.wy = make_float2(wy[0], wy[1]); cp.wz = make_float2(wz[0], wz[1]);
-        a.cells[first_slot / 2 + tid] = cp;
+#pragma unroll
+    for (int u = 0; u < PREP_PER_THREAD; ++u) {
+        const int i = 2 * tid + u;
+        if (i < n_slots) {
+            Cell ce;
+            ce.Y = Y[u]; ce.Z = Z[u];
+            ce.wN = wN[u]; ce.wx = wx[u]; ce.wy = wy[u]; ce.wz = wz[u];
+            a.cells[first_slot + i] = ce;
+        }
     }
 }
 
@@ -135,7 +138,7 @@ nms_status launch_prep(nms_ctx* c)
     a.first_slot = (const int64_t*)base;
     a.flags = (const int32_t*)(base + sizeof(int64_t) * (size_t)c->n_tiles);
     a.meta = (TileMeta*)c->tile_meta.p;
-    a.cells = (CellPair*)c->cells.p;
+    a.cells = (Cell*)c->cells.p;
     a.wsum = (double*)c->wsum.p;
     for (int i = 0; i < 9; ++i) a.R[i] = c->R[i];
     NMS_CUDA(c, cudaMemsetAsync(c->wsum.p, 0, 4 * sizeof(double), c->stream));

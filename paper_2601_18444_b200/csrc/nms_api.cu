@@ -105,7 +105,7 @@ static nms_status build_tiles(nms_ctx* c)
     const size_t bytes = n * (sizeof(TileSrc) + sizeof(int64_t) + sizeof(int32_t));
     if (nms_status st = ensure(c, c->tile_src, bytes)) return st;
     if (nms_status st = ensure(c, c->tile_meta, n * sizeof(TileMeta))) return st;
-    if (nms_status st = ensure(c, c->cells, (size_t)(slot / 2) * sizeof(CellPair))) return st;
+    if (nms_status st = ensure(c, c->cells, (size_t)slot * sizeof(Cell))) return st;
     if (nms_status st = ensure(c, c->wsum, 4 * sizeof(double))) return st;
     char* base = (char*)c->tile_src.p;
     NMS_CUDA(c, cudaMemcpyAsync(base, c->h_tile_src.data(), n * sizeof(TileSrc), cudaMemcpyHostToDevice, c->stream));

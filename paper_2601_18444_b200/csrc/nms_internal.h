@@ -10,25 +10,25 @@ namespace nms {
 
 // ---- packed real-space layout (a-1) ----------------------------------------------------------
 // Cells are grouped into tiles of at most TILE consecutive cells (never straddling an object when
-// an object structure is set).  A tile is stored as CellPair records: two consecutive cells (a, b)
-// side by side, so that every FP32 operation of the amplitude kernel is a packed fma.rn.f32x2 over the
-// pair.  Coordinates are the rotated detector-plane coordinates Y, Z (Eq. 39-40) in fp64 -- the phase
-// is formed in fp64 (one DFMA per pair on the FP64 pipe), see k_amplitude.cu; X is never needed:
-// q_x = 0 (Eq. 41).  Weights are rounded once to fp32.  Odd tiles are padded with a zero-weight cell.
+// an object structure is set).  A tile is an array of 32-byte Cell records.  Coordinates are the
+// rotated detector-plane coordinates Y, Z (Eq. 39-40) in fp64 -- the phase is formed in fp64 (one DFMA
+// per evaluated phasor on the FP64 pipe), see k_amplitude.cu; X is never needed: q_x = 0 (Eq. 41).
+// Weights are rounded once to fp32.  The amplitude kernel keeps each complex accumulator as one packed
+// register pair {sum w cos, sum w sin} and updates it with a single fma.rn.f32x2 {w, w} * {cos, sin} + acc
+// whose first operand is the 32-bit weight register broadcast to both halves (SASS: FFMA2 Rd, Rw.F32, ...),
+// so an accumulation reads one 32-bit and two 64-bit registers.
 constexpr int TILE = 512;
-constexpr int SLOT_PAD = 2;
+constexpr int SLOT_PAD = 1;
 
-struct CellPair {          // 64 B, the unit of the bulk copies (16-byte aligned)
-    double Ya, Yb;         // [nm]
-    double Za, Zb;
-    float2 wN, wx;         // {a, b}: nuclear weight, m'_x
-    float2 wy, wz;         // {a, b}: m'_y, m'_z
+struct Cell {              // 32 B, the unit of the bulk copies (16-byte aligned)
+    double Y, Z;           // [nm]
+    float wN, wx, wy, wz;  // nuclear weight, m'_x, m'_y, m'_z
 };
 
 struct TileMeta {          // consumed by the amplitude kernel
     double Y0, Z0;         // bounding-box midpoint [nm] (origin of the line-recurrence kernel)
-    int64_t first_slot;    // index into the cell array (cells, always even)
-    int32_t n_slots;       // padded cell count (multiple of SLOT_PAD)
+    int64_t first_slot;    // index into the cell array
+    int32_t n_slots;       // cell count of the tile
     int32_t flags;         // bit 0: last tile of its object, bit 1: first tile (form-factor split)
     float ext;             // max over the tile's cells of |Y - Y0|, |Z - Z0| [nm]
     int32_t pad_;
@@ -83,7 +83,7 @@ struct nms_ctx {
     std::vector<nms::TileSrc> h_tile_src;
     std::vector<int32_t> h_tile_flags;
     std::vector<int64_t> h_tile_first_slot;
-    nms::DevBuf tile_src, tile_meta, cells, wsum;   // cells: CellPair[n_slots/2]; wsum: double[4]
+    nms::DevBuf tile_src, tile_meta, cells, wsum;   // cells: Cell[n_slots]; wsum: double[4]
 
     // current detector grid
     bool grid_valid = false;
