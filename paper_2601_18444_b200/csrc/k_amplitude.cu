@@ -4,7 +4,7 @@
 //
 // Work decomposition: grid = (detector blocks) x (cell chunks).  A block owns 128*QT detector points
 // (thread = one position along the fast detector index i1 and QT consecutive positions along i0) and
-// walks the tiles of its chunk.  Tiles (<= 512 Cell records of 32 B) are brought into shared memory by
+// walks the tiles of its chunk.  Tiles (<= TILE = 256 Cell records of 32 B) are brought into shared memory by
 // one elected thread with cp.async.bulk + mbarrier, double buffered; every lane of a warp reads the same
 // record (2 LDS.128 broadcasts per cell, no bank conflicts).
 //
@@ -23,7 +23,7 @@
 //               A complex accumulator is ONE 64-bit register pair, so a detector point costs 8 registers
 //               and a thread with QT = 8 points needs 64 accumulator registers: 4 blocks of 128 threads
 //               per SM (16 warps) instead of 2, which is what hides the MUFU / FP64 / LDS latencies.
-// Accumulators are fp32 over one tile only (<= 512 additions); at the end of a tile they are added to
+// Accumulators are fp32 over one tile only (<= 256 additions); at the end of a tile they are added to
 // fp64 chunk partials in global memory (block-private slots, plain read-modify-write, deterministic).
 // The epilogue kernel sums the chunks and forms the responses.
 //
@@ -140,23 +140,15 @@ __device__ __forceinline__ u64 fmul2(u64 a, u64 b)
 
 // The low word of m holds frac(t) * 2^32 as a signed integer (t = phase in cycles, see MAGIC).  One I2FP
 // (24 significant bits: |error| <= 2^-25 cycle) and one multiply give x = 2 pi frac in [-pi, pi); the
-// phasor {cos x, sin x} comes back as one packed register pair.
+// phasor {cos x, sin x} comes back as one packed register pair.  (sin.approx / cos.approx multiply x by
+// fl(1 / 2 pi) again -- FMUL.RZ, then MUFU on cycles; PTX offers no entry point that skips it.  A relative
+// error of the phase SCALE acts like q -> q (1 + eps), a coherent error of 2 eps q L in the cross sections;
+// measured against the oracle the net scale of this chain is 1 - 1e-8, small enough.)
 __device__ __forceinline__ u64 phasor(double m)
 {
     const float TWO_PI_2M32 = 0x1.921fb6p-30f;   // fl(2 pi) * 2^-32
-#if defined(ABL) && (ABL == 1)
-    const float x = __int2float_rn(__double2loint(m)) * TWO_PI_2M32;
-    return pack2(x, x * 0.5f);
-#elif defined(ABL) && (ABL == 2)
-    const float x = __int_as_float(__double2loint(m)) * TWO_PI_2M32;
-    return pack2(x, x * 0.5f);
-#elif defined(ABL) && (ABL == 4)
-    const float x = __int2float_rn(__double2loint(m)) * TWO_PI_2M32;
-    return pack2(exp2f(x), exp2f(x + 1.0f));
-#else
     const float x = __int2float_rn(__double2loint(m)) * TWO_PI_2M32;
     return pack2(__cosf(x), __sinf(x));
-#endif
 }
 
 // 4 packed accumulations of one (cell, detector point): acc[c] += {w_c, w_c} * {cos, sin}.  The pack of a
@@ -187,11 +179,11 @@ __device__ __forceinline__ void flush_point(const AmpArgs& a, int chunk, int64_t
                                             bool p_first, bool p_last, bool first_total)
 {
     if (!SPLIT) {
+        // fire-and-forget reductions (RED.ADD.F64, no round trip to the thread); the slots are block-private
+        // and zeroed before the launch, so every address sees its additions in tile order: deterministic
+        (void)first;
 #pragma unroll
-        for (int r = 0; r < 8; ++r) {
-            double* dst = a.part + ((int64_t)chunk * 8 + r) * a.n_q + f;
-            *dst = first ? Ap[r] : (*dst + Ap[r]);
-        }
+        for (int r = 0; r < 8; ++r) atomicAdd(a.part + ((int64_t)chunk * 8 + r) * a.n_q + f, Ap[r]);
     } else {
 #pragma unroll
         for (int r = 0; r < 8; ++r) {
@@ -359,11 +351,7 @@ __global__ void __launch_bounds__(AMP_THREADS, MINB) k_amp(const AmpArgs a)
         mbar_wait(&bar[stage], (uint32_t)((it >> 1) & 1));
 
         const int nc = tm.n_slots;
-#if defined(ABL) && (ABL == 3)
-#pragma unroll 1
-#else
-#pragma unroll 2
-#endif
+#pragma unroll 4
         for (int j = 0; j < nc; ++j) {
             const double2 YZ = *reinterpret_cast<const double2*>(&tC[j].Y);
             const float4 w = *reinterpret_cast<const float4*>(&tC[j].wN);
@@ -587,6 +575,8 @@ nms_status launch_amplitude(nms_ctx* c, const AmpPlan& plan, const int32_t* kind
     amp_kernel_t kern = pick_kernel(plan.variant, plan.qt, c->opt_bases, plan.split);
     NMS_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)AMP_SMEM));
     dim3 grid((unsigned)plan.n_qblocks, (unsigned)n_chunks);
+    if (!plan.split)   // the kernel accumulates into its chunk partials with reductions
+        NMS_CUDA(c, cudaMemsetAsync(c->part.p, 0, sizeof(double) * 8 * (size_t)c->n_q * n_chunks, c->stream));
     timer_begin(c, NMS_T_AMPLITUDE);
     kern<<<grid, AMP_THREADS, plan.variant == 8 ? 0 : AMP_SMEM, c->stream>>>(a);
     timer_end(c, NMS_T_AMPLITUDE);

@@ -1,7 +1,7 @@
 // k_prep.cu -- a-1: rotate + pack the real-space sample into tiles, and detector set-up.
 //
 //  prep kernel   (Eq. 37-41):  r' = R (x + r^k), m' = R m in fp64; only Y, Z (rows 2, 3 of R)
-//                are kept because q_x = 0 on the detector (Eq. 41).  One block per tile, two cells per
+//                are kept because q_x = 0 on the detector (Eq. 41).  One block per tile, TILE/256 cells per
 //                thread: it writes the Cell records (fp64 Y, Z; weights rounded once to fp32), finds
 //                the tile's bounding-box midpoint (Y0, Z0) and extent, and accumulates sum_j |w_cj| for
 //                the tolerance denominators.
@@ -65,7 +65,7 @@ __global__ void __launch_bounds__(PREP_THREADS) k_prep(const PrepArgs a)
     double sN = 0.0, sx = 0.0, sy = 0.0, sz = 0.0;
 #pragma unroll
     for (int u = 0; u < PREP_PER_THREAD; ++u) {
-        const int i = 2 * tid + u;
+        const int i = PREP_PER_THREAD * tid + u;
         Y[u] = Z[u] = 0.0;
         wN[u] = wx[u] = wy[u] = wz[u] = 0.f;
         if (i < ts.n_src) {
@@ -115,7 +115,7 @@ __global__ void __launch_bounds__(PREP_THREADS) k_prep(const PrepArgs a)
     }
 #pragma unroll
     for (int u = 0; u < PREP_PER_THREAD; ++u) {
-        const int i = 2 * tid + u;
+        const int i = PREP_PER_THREAD * tid + u;
         if (i < n_slots) {
             Cell ce;
             ce.Y = Y[u]; ce.Z = Z[u];

@@ -17,7 +17,7 @@ namespace nms {
 // register pair {sum w cos, sum w sin} and updates it with a single fma.rn.f32x2 {w, w} * {cos, sin} + acc
 // whose first operand is the 32-bit weight register broadcast to both halves (SASS: FFMA2 Rd, Rw.F32, ...),
 // so an accumulation reads one 32-bit and two 64-bit registers.
-constexpr int TILE = 512;
+constexpr int TILE = 256;
 constexpr int SLOT_PAD = 1;
 
 struct Cell {              // 32 B, the unit of the bulk copies (16-byte aligned)
