@@ -134,6 +134,20 @@ def azimuthal_polar(maps, n0: int, n1: int):
     return out
 
 
+def modal(maps, n0: int, n1: int, theta, k_max: int):
+    """Angular modal decomposition (Eq. 31-33) of maps [n_maps, n0*n1] on a polar grid with angles theta [n1]:
+    returns (Is, Ic) [n_maps, k_max+1, n0], (a_s, a_c) and (A_s, A_c) [n_maps, k_max+1]."""
+    maps = _f64(maps).reshape(-1, n0 * n1)
+    theta = _f64(theta)
+    nm, nk = maps.shape[0], k_max + 1
+    Is, Ic = np.empty((nm, nk, n0)), np.empty((nm, nk, n0))
+    a_s, a_c, A_s, A_c = (np.empty((nm, nk)) for _ in range(4))
+    _chk(lib().nmso_modal(_p(maps, C.c_double), C.c_int(nm), C.c_int(n0), C.c_int(n1), _p(theta, C.c_double),
+                          C.c_int(k_max), _p(Is, C.c_double), _p(Ic, C.c_double), _p(a_s, C.c_double),
+                          _p(a_c, C.c_double), _p(A_s, C.c_double), _p(A_c, C.c_double)), "modal")
+    return Is, Ic, a_s, a_c, A_s, A_c
+
+
 def azimuthal_hist(maps, qy, qz, n_bins: int, q_lo: float, q_hi: float):
     """(I [n_maps, n_bins], count [n_bins]) histogram means by |q| (reading 8)."""
     qy, qz = _f64(qy), _f64(qz)

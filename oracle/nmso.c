@@ -20,7 +20,9 @@
  * Eq. 9/15/28, uniform-m angular factors Eq. 60-63, Table II I(0)
  * values, sphere form factor, azimuthal means Eq. 65-67, Fourier-Bessel
  * of the sphere form factor (gamma_0), form/interference split of two
- * identical particles.  No function here is "parity unpinned".
+ * identical particles, angular modal decomposition of trigonometric maps
+ * (A_0^c / A_2^c = -1 for sin^2, A_0^c / A_4^c = -1 for sin^2 cos^2, L199).
+ * No function here is "parity unpinned".
  *
  * Build: gcc -O2 -fopenmp -shared -fPIC -o libnmso.so nmso.c -lm
  */
@@ -305,6 +307,51 @@ int nmso_form_factor_split(const float *pos, const float *N, const float *m, int
     if (!rc) rc = nmso_response(At, theta, nq, P, sN, sM, invV, kinds, nk, out_total, NULL);
     free(Ap); free(At); free(Bp);
     return rc;
+}
+
+/* ------------------------------------------------------------------------
+ * Angular modal decomposition, Eq. 31-33 (L187-L199).  On a polar grid with
+ * theta_j = 2 pi j / n_theta (reading 7) the trapezoidal rule of Eq. 31
+ * is the plain sum
+ *   I_k^{s,c}(q_i) = (2 - delta_k0) / n_theta * sum_j f(q_i, theta_j) {sin, cos}(k theta_j),
+ * with theta_j the grid's own (float32, promoted) angles.  Eq. 32: a_k = sum_i I_k(q_i).
+ * Eq. 33: A_k = a_k / sum_{j=0..kmax} sqrt(a_j^s^2 + a_j^c^2) (0 where that sum is 0).
+ * maps [nm][n0][n1]; Is, Ic [nm][kmax+1][n0]; as_, ac, As, Ac [nm][kmax+1].
+ * ---------------------------------------------------------------------- */
+int nmso_modal(const double *maps, int nm, int n0, int n1, const double *theta, int kmax,
+               double *Is, double *Ic, double *as_, double *ac, double *As, double *Ac)
+{
+    if (!maps || !theta || !Is || !Ic || !as_ || !ac || !As || !Ac || nm <= 0 || n0 <= 0 || n1 <= 0 || kmax < 0)
+        return NMSO_E_ARG;
+    const int nk = kmax + 1;
+    for (int a = 0; a < nm; ++a) {
+        for (int k = 0; k < nk; ++k) {
+            const double pref = (k == 0 ? 1.0 : 2.0) / (double)n1;
+            double sa = 0.0, ca = 0.0;
+            for (int i = 0; i < n0; ++i) {
+                double ss = 0.0, cc = 0.0;
+                for (int j = 0; j < n1; ++j) {
+                    const double f = maps[((int64_t)a * n0 + i) * n1 + j];
+                    ss += f * sin((double)k * theta[j]);
+                    cc += f * cos((double)k * theta[j]);
+                }
+                Is[((int64_t)a * nk + k) * n0 + i] = pref * ss;
+                Ic[((int64_t)a * nk + k) * n0 + i] = pref * cc;
+                sa += pref * ss;
+                ca += pref * cc;
+            }
+            as_[(int64_t)a * nk + k] = sa;
+            ac[(int64_t)a * nk + k] = ca;
+        }
+        double norm = 0.0;
+        for (int k = 0; k < nk; ++k)
+            norm += sqrt(as_[(int64_t)a * nk + k] * as_[(int64_t)a * nk + k] + ac[(int64_t)a * nk + k] * ac[(int64_t)a * nk + k]);
+        for (int k = 0; k < nk; ++k) {
+            As[(int64_t)a * nk + k] = norm > 0.0 ? as_[(int64_t)a * nk + k] / norm : 0.0;
+            Ac[(int64_t)a * nk + k] = norm > 0.0 ? ac[(int64_t)a * nk + k] / norm : 0.0;
+        }
+    }
+    return NMSO_OK;
 }
 
 /* ------------------------------------------------------------------------

@@ -540,3 +540,83 @@ def test_generator_cell_counts_and_table1_rows():
     w5 = ni.make_config("C5", small=True)
     assert 0.05 <= np.mean(w5.N == 0) < 0.06
     np.testing.assert_allclose(np.linalg.norm(w5.m.astype(np.float64), axis=1), 1.0, atol=1e-6)
+
+
+# ----------------------------------------------------------------------------------------------------
+# angular modal decomposition, Eq. 31-33 (L187-L199)
+# ----------------------------------------------------------------------------------------------------
+def _theta(n):
+    return (2.0 * np.pi * np.arange(n) / n).astype(np.float32).astype(np.float64)
+
+
+def test_modal_two_and_four_fold_anisotropy_ratios(oracle_mod):
+    """L199: 'a two-fold sin^2 theta anisotropy yields A_0^c / A_2^c = -1, whereas for the case of a four-fold
+    sin^2 theta cos^2 theta anisotropy A_0^c / A_4^c = -1' -- sin^2 = (1 - cos 2 theta)/2 and
+    sin^2 cos^2 = (1 - cos 4 theta)/8, so I_0^c = u/2, I_2^c = -u/2 resp. I_0^c = u/8, I_4^c = -u/8."""
+    n0, n1, kmax = 7, 48, 6
+    th = _theta(n1)
+    u = np.linspace(1.0, 3.0, n0)
+    f2 = (u[:, None] * np.sin(th)[None, :] ** 2).reshape(1, -1)
+    f4 = (u[:, None] * (np.sin(th) * np.cos(th))[None, :] ** 2).reshape(1, -1)
+    Is, Ic, a_s, a_c, A_s, A_c = oracle_mod.modal(np.concatenate([f2, f4]), n0, n1, th, kmax)
+    np.testing.assert_allclose(Ic[0, 0], u / 2, rtol=1e-6)
+    np.testing.assert_allclose(Ic[0, 2], -u / 2, rtol=1e-6)
+    np.testing.assert_allclose(Ic[1, 0], u / 8, rtol=1e-6)
+    np.testing.assert_allclose(Ic[1, 4], -u / 8, rtol=1e-6)
+    assert A_c[0, 0] / A_c[0, 2] == pytest.approx(-1.0, rel=1e-6)
+    assert A_c[1, 0] / A_c[1, 4] == pytest.approx(-1.0, rel=1e-6)
+    other2 = [k for k in range(kmax + 1) if k not in (0, 2)]
+    assert np.abs(Ic[0][other2]).max() < 1e-6 and np.abs(Is[0]).max() < 1e-6
+    # Eq. 32-33: a_k = sum_i I_k(q_i); A_k normalised by sum_j sqrt(a_j^s^2 + a_j^c^2)
+    np.testing.assert_allclose(a_c[0, 0], u.sum() / 2, rtol=1e-6)
+    np.testing.assert_allclose(np.sqrt(A_s ** 2 + A_c ** 2).sum(axis=1), 1.0, rtol=1e-12)
+
+
+def test_modal_recovers_a_trigonometric_polynomial(oracle_mod):
+    """f = c0 + sum_k (c_k cos k theta + s_k sin k theta), k <= 5 < n_theta / 2: Eq. 31 by the periodic trapezoid
+    returns exactly I_0^c = c0, I_k^c = c_k, I_k^s = s_k (prefactor (2 - delta_k0) / 2 pi); the fp32 rounding of
+    the grid's theta_j limits the agreement to ~k * 2^-24 * 2 pi."""
+    rng = np.random.Generator(np.random.Philox(31))
+    n0, n1, kmax = 3, 40, 5
+    th = _theta(n1)
+    c = rng.normal(size=(n0, kmax + 1))
+    s = rng.normal(size=(n0, kmax + 1)); s[:, 0] = 0.0
+    f = sum(c[:, k, None] * np.cos(k * th)[None, :] + s[:, k, None] * np.sin(k * th)[None, :] for k in range(kmax + 1))
+    Is, Ic, a_s, a_c, A_s, A_c = oracle_mod.modal(f.reshape(1, -1), n0, n1, th, kmax)
+    np.testing.assert_allclose(Ic[0].T, c, atol=2e-5)
+    np.testing.assert_allclose(Is[0].T, s, atol=2e-5)
+    np.testing.assert_allclose(a_c[0], c.sum(axis=0), atol=1e-4)
+    np.testing.assert_allclose(a_s[0], s.sum(axis=0), atol=1e-4)
+
+
+def test_modal_order_zero_is_the_azimuthal_average_and_brute_force(oracle_mod):
+    """k = 0 of Eq. 31 is Eq. 30; every entry against a literal Python loop on a random map."""
+    rng = np.random.Generator(np.random.Philox(32))
+    n0, n1, kmax = 4, 17, 3
+    th = _theta(n1)
+    f = rng.normal(size=(2, n0 * n1))
+    Is, Ic, a_s, a_c, A_s, A_c = oracle_mod.modal(f, n0, n1, th, kmax)
+    np.testing.assert_allclose(Ic[:, 0], oracle_mod.azimuthal_polar(f, n0, n1), rtol=1e-13, atol=1e-15)
+    for a in range(2):
+        for k in range(kmax + 1):
+            for i in range(n0):
+                ss = sum(f[a, i * n1 + j] * math.sin(k * th[j]) for j in range(n1))
+                cc = sum(f[a, i * n1 + j] * math.cos(k * th[j]) for j in range(n1))
+                pref = (1.0 if k == 0 else 2.0) / n1
+                assert Is[a, k, i] == pytest.approx(pref * ss, rel=1e-12, abs=1e-14)
+                assert Ic[a, k, i] == pytest.approx(pref * cc, rel=1e-12, abs=1e-14)
+        norm = sum(math.hypot(Is[a, k].sum(), Ic[a, k].sum()) for k in range(kmax + 1))
+        np.testing.assert_allclose(A_c[a], Ic[a].sum(axis=1) / norm, rtol=1e-12)
+        np.testing.assert_allclose(A_s[a], Is[a].sum(axis=1) / norm, rtol=1e-12, atol=1e-15)
+
+
+def test_modal_uniform_sphere_magnetic_channel(oracle_mod):
+    """C1-type sample (uniform m = e_z): MAG = |F|^2 sin^2 theta (Eq. 60) up to the lattice's own weak angular
+    dependence, hence A_0^c / A_2^c = -1 to that level and all sine amplitudes vanish (mirror symmetry)."""
+    wl = ni.make_config("C1")
+    qy, qz, th = oracle_mod.grid_points(wl.grid)
+    A = oracle_mod.amplitudes(wl.pos, wl.N, wl.m, wl.R, qy, qz)
+    M = oracle_mod.response(A, th, [KI["MAG"]], P=wl.P)
+    Is, Ic, a_s, a_c, A_s, A_c = oracle_mod.modal(M, wl.grid.n0, wl.grid.n1, wl.grid.u1, 4)
+    assert A_c[0, 0] / A_c[0, 2] == pytest.approx(-1.0, abs=0.02)
+    assert np.abs(A_s[0]).max() < 1e-6
