@@ -92,7 +92,8 @@ typedef enum {
     NMS_T_EPILOGUE = 2,     /* a-3 reduce + responses                               */
     NMS_T_AZIMUTHAL = 3,    /* a-4                                                  */
     NMS_T_CORRELATION = 4,  /* a-5                                                  */
-    NMS_T_COUNT = 5
+    NMS_T_MODAL = 5,        /* f-2 angular modal decomposition                      */
+    NMS_T_COUNT = 6
 } nms_timer;
 
 /* ---- context ---------------------------------------------------------------------------------- */
@@ -157,6 +158,18 @@ NMS_API nms_status nms_compute(nms_ctx* ctx, const nms_qgrid* grid, const nms_ki
 NMS_API nms_status nms_azimuthal_average(nms_ctx* ctx, const float* maps, int n_maps, int n_bins, double q_lo,
                                  double q_hi, float* out_I, float* out_q, int32_t* out_count);
 
+/* ---- angular modal decomposition (f-2, Eq. 31-33) -------------------------------------- */
+
+/* Sine and cosine harmonics of maps [dev][n_maps][n_q] (float) on the context's current grid, which must be
+ * polar with theta_j = 2 pi j / n1 (reading 7; NMS_E_UNSUPPORTED otherwise): for k = 0..k_max (k_max <= 63)
+ *   I_k^{s,c}(q_i) = (2 - delta_k0) / n1 * sum_j f(q_i, theta_j) {sin, cos}(k theta_j)      (Eq. 31, trapezoid L183)
+ *   a_k^{s,c} = sum_i I_k^{s,c}(q_i)                                                        (Eq. 32)
+ *   A_k^{s,c} = a_k^{s,c} / sum_{j=0..k_max} sqrt(a_j^s^2 + a_j^c^2)   (0 if that sum is 0) (Eq. 33)
+ * in fp64, outputs rounded once to float.  out_Is, out_Ic [dev][n_maps][k_max+1][n0]; out_a, out_A
+ * [dev][n_maps][2][k_max+1] with index 0 = sine, 1 = cosine.  Any output may be NULL (not all).        */
+NMS_API nms_status nms_modal_decomposition(nms_ctx* ctx, const float* maps, int n_maps, int k_max, float* out_Is,
+                                   float* out_Ic, float* out_a, float* out_A);
+
 /* ---- correlation function (a-5, Eq. 34-35) -------------------------------------------- */
 
 /* c(r_k) = (1/2pi^2) trapz_q[ I(q) j0(q r_k) q^2 ], p(r_k) = r_k^2 c(r_k), for each of n_maps curves
@@ -194,14 +207,17 @@ NMS_API nms_status nms_run_host(nms_ctx* ctx, const float* pos, const float* N, 
  * the amplitude tolerance 1e-5 sum|w|); synchronises.                                            */
 NMS_API nms_status nms_get_weight_sums(nms_ctx* ctx, double* out);
 
-/* Integer options.  "variant": 0 auto, 1 force the direct (MUFU per pair) kernel, 2 force the
- * recurrence kernel (NMS_E_UNSUPPORTED at compute time if the detector lines are not equally spaced).
- * "timing": 1 records a CUDA event pair around every kernel launch (and resets the record).  "chunks": 0 auto, else the number of cell
- * chunks.  "qt": 0 auto, else detector points per thread (4, 8 or 16).  Unknown keys: NMS_E_ARG. */
+/* Integer options.  "variant": 0 auto (exact fp64 kernel for W * n_q <= 2^30, else the line-recurrence
+ * kernel where u0 is equally spaced, else the direct kernel), 1 force the direct (MUFU per pair) kernel,
+ * 2 force the line-recurrence kernel (NMS_E_UNSUPPORTED at compute time if the detector is a point list or
+ * u0 is not an arithmetic progression within one fp32 ulp), 3 force the exact fp64 kernel.  "bases": exactly
+ * evaluated points per 8 in the recurrence kernel (0 auto = 2, else 1..4).  "timing": 1 records a CUDA
+ * event pair around every kernel launch (and resets the record).  "chunks": 0 auto, else the number of cell
+ * chunks.  "qt": 0 auto, else detector points per thread (4 or 8).  Unknown keys: NMS_E_ARG.            */
 NMS_API nms_status nms_set_option(nms_ctx* ctx, const char* key, int64_t value);
-/* Read back integers: "launches" (kernels launched by this context so far), "variant_used" (1 general
- * direct, 2 polar direct, 4 cartesian direct, 3 line recurrence), "n_chunks", "n_tiles", "n_slots",
- * "sm_count", "blocks_per_sm", "qt".                                                             */
+/* Read back integers: "launches" (kernels launched by this context so far), "variant_used" (1 list direct,
+ * 2 polar direct, 4 cartesian direct, 3 polar recurrence, 5 cartesian recurrence, 8 exact fp64),
+ * "n_chunks", "n_tiles", "n_slots", "sm_count", "blocks_per_sm", "qt".                              */
 NMS_API nms_status nms_get_info(nms_ctx* ctx, const char* key, int64_t* value);
 /* Device time in ms of the most recent launch of the given kernel class ("timing" must be 1);
  * synchronises on that kernel's end event.  NMS_E_STATE if it has not run.                       */

@@ -26,14 +26,14 @@ LIB_PATH = os.path.join(_HERE, "libnms.so")
 
 KINDS = ["NUC", "MAG", "UNPOL", "PROJ", "NM", "SF", "CHI", "PM", "MP", "PP", "MM", "POL_PLUS", "POL_MINUS"]
 NMS_OK, NMS_E_ARG, NMS_E_STATE, NMS_E_CUDA, NMS_E_NOMEM, NMS_E_UNSUPPORTED = range(6)
-NMS_T_PREP, NMS_T_AMPLITUDE, NMS_T_EPILOGUE, NMS_T_AZIMUTHAL, NMS_T_CORRELATION = range(5)
+NMS_T_PREP, NMS_T_AMPLITUDE, NMS_T_EPILOGUE, NMS_T_AZIMUTHAL, NMS_T_CORRELATION, NMS_T_MODAL = range(6)
 _STATUS = {0: "NMS_OK", 1: "NMS_E_ARG", 2: "NMS_E_STATE", 3: "NMS_E_CUDA", 4: "NMS_E_NOMEM", 5: "NMS_E_UNSUPPORTED"}
 
 EXPORTS = [
     "nms_create", "nms_destroy", "nms_last_error", "nms_synchronize", "nms_set_sample", "nms_set_particles",
     "nms_set_rotation", "nms_set_polarization", "nms_set_scales", "nms_amplitudes", "nms_response", "nms_compute",
     "nms_azimuthal_average", "nms_correlation", "nms_form_factor_split", "nms_run_host", "nms_get_weight_sums",
-    "nms_set_option", "nms_get_info", "nms_kernel_time_ms", "nms_kernel_time_total",
+    "nms_set_option", "nms_get_info", "nms_kernel_time_ms", "nms_kernel_time_total", "nms_modal_decomposition",
 ]
 
 
@@ -180,6 +180,11 @@ def nms_form_factor_split(ctx, grid, kinds, out_total, out_form):
 def nms_azimuthal_average(ctx, maps, n_maps, n_bins, q_lo, q_hi, out_I, out_q=None, out_count=None):
     _check(ctx, _lib.nms_azimuthal_average(ctx, _dev(maps), C.c_int(n_maps), C.c_int(n_bins), C.c_double(q_lo),
                                            C.c_double(q_hi), _dev(out_I), _dev(out_q), _dev(out_count)))
+
+
+def nms_modal_decomposition(ctx, maps, n_maps, k_max, out_Is=None, out_Ic=None, out_a=None, out_A=None):
+    _check(ctx, _lib.nms_modal_decomposition(ctx, _dev(maps), C.c_int(n_maps), C.c_int(k_max), _dev(out_Is), _dev(out_Ic),
+                                             _dev(out_a), _dev(out_A)))
 
 
 def nms_correlation(ctx, I, q_of_bin, count, n_maps, n_bins, r, out_c, out_p):

@@ -351,7 +351,7 @@ __global__ void __launch_bounds__(AMP_THREADS, MINB) k_amp(const AmpArgs a)
         mbar_wait(&bar[stage], (uint32_t)((it >> 1) & 1));
 
         const int nc = tm.n_slots;
-#pragma unroll 4
+#pragma unroll 8
         for (int j = 0; j < nc; ++j) {
             const double2 YZ = *reinterpret_cast<const double2*>(&tC[j].Y);
             const float4 w = *reinterpret_cast<const float4*>(&tC[j].wN);

@@ -27,6 +27,110 @@ __global__ void __launch_bounds__(256) k_ring_mean(const float* __restrict__ map
     }
 }
 
+// ---- angular modal decomposition (Eq. 31-33) -------------------------------
+// I_k^{s,c}(q_i) = (2 - delta_k0) / n_theta * sum_j f(q_i, theta_j) {sin, cos}(k theta_j): the trapezoidal rule
+// of L183 on the periodic theta grid (reading 7).  Pass 1 tabulates (sin, cos)(k theta_j) in fp64 from the
+// grid's own float angles; pass 2 is one warp per (map, k, ring) with fp64 partial sums and warp shuffles;
+// pass 3 (one block per map, one warp per k) forms a_k = sum_i I_k(q_i) (Eq. 32) from the fp64 ring values
+// and A_k = a_k / sum_j sqrt(a_j^s^2 + a_j^c^2) (Eq. 33).
+__global__ void k_modal_table(const float* __restrict__ theta, int n1, int nk, double2* __restrict__ tab)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= nk * n1) return;
+    const int k = t / n1, j = t % n1;
+    double s, c;
+    sincos((double)k * (double)theta[j], &s, &c);
+    tab[t] = make_double2(s, c);
+}
+
+__global__ void __launch_bounds__(256) k_modal_rings(const float* __restrict__ maps, int n_maps, int n0, int n1, int nk,
+                                                     const double2* __restrict__ tab, double2* __restrict__ ring,
+                                                     float* __restrict__ out_Is, float* __restrict__ out_Ic)
+{
+    const int64_t w = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;   // (map, k, ring)
+    const int lane = threadIdx.x & 31;
+    if (w >= (int64_t)n_maps * nk * n0) return;
+    const int i = (int)(w % n0), k = (int)((w / n0) % nk), a = (int)(w / ((int64_t)n0 * nk));
+    const float* row = maps + ((int64_t)a * n0 + i) * n1;
+    const double2* tk = tab + (int64_t)k * n1;
+    double ss = 0.0, cc = 0.0;
+    for (int j = lane; j < n1; j += 32) {
+        const double f = (double)row[j];
+        const double2 sc = tk[j];
+        ss = fma(f, sc.x, ss);
+        cc = fma(f, sc.y, cc);
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        ss += __shfl_xor_sync(0xffffffffu, ss, o);
+        cc += __shfl_xor_sync(0xffffffffu, cc, o);
+    }
+    if (lane == 0) {
+        const double pref = (k == 0 ? 1.0 : 2.0) / (double)n1;
+        ss *= pref; cc *= pref;
+        ring[w] = make_double2(ss, cc);
+        if (out_Is) out_Is[w] = (float)ss;
+        if (out_Ic) out_Ic[w] = (float)cc;
+    }
+}
+
+constexpr int MODAL_KMAX = 63;
+
+__global__ void __launch_bounds__(1024) k_modal_amplitudes(const double2* __restrict__ ring, int n0, int nk,
+                                                           float* __restrict__ out_a, float* __restrict__ out_A)
+{
+    __shared__ double as_[MODAL_KMAX + 1], ac_[MODAL_KMAX + 1];
+    __shared__ double norm;
+    const int a = blockIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5, n_warps = blockDim.x >> 5;
+    for (int k = warp; k < nk; k += n_warps) {
+        const double2* r = ring + ((int64_t)a * nk + k) * n0;
+        double ss = 0.0, cc = 0.0;
+        for (int i = lane; i < n0; i += 32) { ss += r[i].x; cc += r[i].y; }
+        for (int o = 16; o > 0; o >>= 1) {
+            ss += __shfl_xor_sync(0xffffffffu, ss, o);
+            cc += __shfl_xor_sync(0xffffffffu, cc, o);
+        }
+        if (lane == 0) { as_[k] = ss; ac_[k] = cc; }
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double n = 0.0;
+        for (int k = 0; k < nk; ++k) n += sqrt(as_[k] * as_[k] + ac_[k] * ac_[k]);
+        norm = n;
+    }
+    __syncthreads();
+    for (int k = threadIdx.x; k < nk; k += blockDim.x) {
+        const int64_t o = (int64_t)a * 2 * nk;
+        if (out_a) { out_a[o + k] = (float)as_[k]; out_a[o + nk + k] = (float)ac_[k]; }
+        if (out_A) {
+            out_A[o + k] = norm > 0.0 ? (float)(as_[k] / norm) : 0.f;
+            out_A[o + nk + k] = norm > 0.0 ? (float)(ac_[k] / norm) : 0.f;
+        }
+    }
+}
+
+nms_status launch_modal(nms_ctx* c, const float* maps, int n_maps, int k_max, float* out_Is, float* out_Ic, float* out_a,
+                        float* out_A)
+{
+    const int nk = k_max + 1, n0 = c->g_n0, n1 = c->g_n1;
+    if (nms_status st = ensure(c, c->modal_tab, sizeof(double2) * (size_t)nk * n1)) return st;
+    if (nms_status st = ensure(c, c->modal_ring, sizeof(double2) * (size_t)n_maps * nk * n0)) return st;
+    timer_begin(c, NMS_T_MODAL);
+    k_modal_table<<<(unsigned)((nk * n1 + 255) / 256), 256, 0, c->stream>>>((const float*)c->u1.p, n1, nk,
+                                                                           (double2*)c->modal_tab.p);
+    const int64_t warps = (int64_t)n_maps * nk * n0;
+    k_modal_rings<<<(unsigned)((warps * 32 + 255) / 256), 256, 0, c->stream>>>(maps, n_maps, n0, n1, nk,
+                                                                              (const double2*)c->modal_tab.p,
+                                                                              (double2*)c->modal_ring.p, out_Is, out_Ic);
+    c->launches += 2;
+    if (out_a || out_A) {
+        k_modal_amplitudes<<<(unsigned)n_maps, 1024, 0, c->stream>>>((const double2*)c->modal_ring.p, n0, nk, out_a, out_A);
+        c->launches += 1;
+    }
+    timer_end(c, NMS_T_MODAL);
+    NMS_CUDA(c, cudaGetLastError());
+    return NMS_OK;
+}
+
 // ---- |q| histogram (reading 8) ---------------------------------------------------------------------
 // bin = floor((|q| - q_lo) / (q_hi - q_lo) * n_bins), |q| = sqrt(q_y^2 + q_z^2), in fp64 in exactly this
 // order with individually rounded operations (no FMA contraction): the bin is an integer decision.

@@ -245,7 +245,7 @@ void nms_destroy(nms_ctx* c)
     cudaStreamSynchronize(c->stream);
     DevBuf* bufs[] = {&c->raw_pos, &c->raw_N, &c->raw_m, &c->centres, &c->tile_src, &c->tile_meta, &c->cells,
                       &c->wsum, &c->u0, &c->u1, &c->qc, &c->sc, &c->amp64, &c->part, &c->ppart, &c->formpart,
-                      &c->chunk_begin, &c->kinds_dev, &c->bin_idx, &c->bin_sum, &c->bin_cnt};
+                      &c->chunk_begin, &c->kinds_dev, &c->bin_idx, &c->bin_sum, &c->bin_cnt, &c->modal_tab, &c->modal_ring};
     for (DevBuf* b : bufs) free_buf(*b);
     for (DevBuf& b : c->host_stage) free_buf(b);
     for (Timer& t : c->timers) {
@@ -392,6 +392,18 @@ nms_status nms_azimuthal_average(nms_ctx* c, const float* maps, int n_maps, int 
     return launch_azimuthal(c, maps, n_maps, n_bins, q_lo, q_hi, out_I, out_q, out_count);
 }
 
+nms_status nms_modal_decomposition(nms_ctx* c, const float* maps, int n_maps, int k_max, float* out_Is, float* out_Ic,
+                                   float* out_a, float* out_A)
+{
+    CHECK_CTX(c);
+    if (!c->grid_valid) return fail(c, NMS_E_STATE, "nms_modal_decomposition needs a current grid (nms_amplitudes / nms_compute)");
+    if (c->g_type != 0) return fail(c, NMS_E_UNSUPPORTED, "nms_modal_decomposition needs a polar grid");
+    if (!maps || n_maps <= 0) return fail(c, NMS_E_ARG, "maps NULL or n_maps <= 0");
+    if (k_max < 0 || k_max > 63) return fail(c, NMS_E_ARG, "k_max = %d outside 0..63", k_max);
+    if (!out_Is && !out_Ic && !out_a && !out_A) return fail(c, NMS_E_ARG, "no output requested");
+    return launch_modal(c, maps, n_maps, k_max, out_Is, out_Ic, out_a, out_A);
+}
+
 nms_status nms_correlation(nms_ctx* c, const float* I, const float* q_of_bin, const int32_t* count, int n_maps, int n_bins,
                            const float* r, int n_r, float* out_c, float* out_p)
 {
@@ -457,7 +469,7 @@ nms_status nms_set_option(nms_ctx* c, const char* key, int64_t value)
     else if (!strcmp(key, "timing")) { c->opt_timing = value != 0; for (Timer& t : c->timers) t.used = 0; }
     else if (!strcmp(key, "chunks")) { if (value < 0) return fail(c, NMS_E_ARG, "chunks must be >= 0"); c->opt_chunks = (int)value; }
     else if (!strcmp(key, "bases")) { if (value < 0 || value > 4) return fail(c, NMS_E_ARG, "bases must be 0..4"); c->opt_bases = (int)value; }
-    else if (!strcmp(key, "qt")) { if (value != 0 && value != 4 && value != 8 && value != 16) return fail(c, NMS_E_ARG, "qt must be 0, 4, 8 or 16"); c->opt_qt = (int)value; }
+    else if (!strcmp(key, "qt")) { if (value != 0 && value != 4 && value != 8) return fail(c, NMS_E_ARG, "qt must be 0, 4 or 8"); c->opt_qt = (int)value; }
     else return fail(c, NMS_E_ARG, "unknown option '%s'", key);
     return NMS_OK;
 }

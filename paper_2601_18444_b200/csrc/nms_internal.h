@@ -102,6 +102,7 @@ struct nms_ctx {
     std::vector<int32_t> h_chunk_begin;
     nms::DevBuf kinds_dev;             // int32 [<=13]
     nms::DevBuf bin_idx, bin_sum, bin_cnt;
+    nms::DevBuf modal_tab, modal_ring; // (sin, cos)(k theta_j) table; fp64 ring values of the modal decomposition
     nms::DevBuf host_stage[8];         // device staging for nms_run_host
 
     nms::Timer timers[NMS_T_COUNT];
@@ -145,6 +146,8 @@ nms_status launch_split_epilogue(nms_ctx* c, int n_chunks, const int32_t* kinds_
 // k_post.cu
 nms_status launch_azimuthal(nms_ctx* c, const float* maps, int n_maps, int n_bins, double q_lo, double q_hi,
                             float* out_I, float* out_q, int32_t* out_count);
+nms_status launch_modal(nms_ctx* c, const float* maps, int n_maps, int k_max, float* out_Is, float* out_Ic, float* out_a,
+                        float* out_A);
 nms_status launch_correlation(nms_ctx* c, const float* I, const float* q_of_bin, const int32_t* count, int n_maps,
                               int n_bins, const float* r, int n_r, float* out_c, float* out_p);
 

@@ -377,6 +377,74 @@ def test_azimuthal_and_correlation(nms, ctx, oracle_mod, name):
     assert_cross_sections(p.cpu().numpy(), p_ref, kinds, name + " p(r)")
 
 
+@pytest.mark.parametrize("name,small,k_max", [("C1", False, 6), ("C5", True, 8), ("C3", True, 0), ("C5", True, 63)])
+def test_modal_decomposition(nms, ctx, oracle_mod, name, small, k_max):
+    """f-2, Eq. 31-33: pass-isolated (oracle applied to the GPU's own maps: fp32 output rounding only) and end to
+    end against the oracle's maps; the chiral map's sine harmonics are the reason the paper has this pass (L183)."""
+    import torch
+    wl = ni.make_config(name, small=small)
+    kinds = list(ni.ALL_KINDS)
+    _upload(nms, ctx, wl)
+    n0, n1, nk, nm = wl.grid.n0, wl.grid.n1, k_max + 1, len(kinds)
+    maps = torch.empty((nm, wl.grid.n_q), dtype=torch.float32, device="cuda")
+    nms.nms_compute(ctx, wl.grid, kinds, maps)
+    Is = torch.empty((nm, nk, n0), dtype=torch.float32, device="cuda")
+    Ic = torch.empty_like(Is)
+    a = torch.empty((nm, 2, nk), dtype=torch.float32, device="cuda")
+    A = torch.empty_like(a)
+    nms.nms_modal_decomposition(ctx, maps, nm, k_max, Is, Ic, a, A)
+    nms.nms_synchronize(ctx)
+    maps_h = maps.cpu().numpy()
+    rIs, rIc, ras, rac, rAs, rAc = oracle_mod.modal(maps_h, n0, n1, wl.grid.u1, k_max)
+    scale = np.abs(maps_h).max(axis=1)[:, None, None]              # |I_k| <= 2 max|f|
+    for got, want in ((Is.cpu().numpy(), rIs), (Ic.cpu().numpy(), rIc)):
+        assert np.all(np.abs(got - want) <= 1e-6 * np.abs(want) + 1e-9 * scale)
+    ascale = np.maximum(np.abs(ras), np.abs(rac)).max(axis=1)[:, None]
+    a_h, A_h = a.cpu().numpy(), A.cpu().numpy()
+    assert np.all(np.abs(a_h[:, 0] - ras) <= 1e-6 * np.abs(ras) + 1e-9 * ascale)
+    assert np.all(np.abs(a_h[:, 1] - rac) <= 1e-6 * np.abs(rac) + 1e-9 * ascale)
+    assert np.all(np.abs(A_h[:, 0] - rAs) <= 2e-7) and np.all(np.abs(A_h[:, 1] - rAc) <= 2e-7)   # |A| <= 1
+    # end to end: harmonics of the oracle's own maps; an absolute criterion on the scale of the map
+    qy, qz, th = oracle_mod.grid_points(wl.grid)
+    _, _, M = _oracle_maps(oracle_mod, wl, qy, qz, th, kinds)
+    eIs, eIc, eas, eac, eAs, eAc = oracle_mod.modal(M, n0, n1, wl.grid.u1, k_max)
+    ring_scale = np.abs(M).reshape(nm, n0, n1).max(axis=2)[:, None, :]   # per ring: |I_k(q_i)| <= 2 max_j |f(q_i, .)|
+    fp32 = nms.nms_get_info(ctx, "variant_used") != 8
+    # a harmonic is a mean over the ring with weights of modulus <= 2: maps that are pointwise within the north-star
+    # 1e-3 (MUFU kernels; the exact kernel leaves only the fp32 rounding of the stored maps) give harmonics within
+    # 2 tol max_j |f(q_i, theta_j)|
+    tol = 1e-3 if fp32 else 2e-7
+    assert np.all(np.abs(Ic.cpu().numpy() - eIc) <= 2 * tol * ring_scale)
+    assert np.all(np.abs(Is.cpu().numpy() - eIs) <= 2 * tol * ring_scale)
+    np.testing.assert_allclose(A_h[:, 1, 0], eAc[:, 0], rtol=1e-3, atol=1e-6)
+
+
+def test_modal_decomposition_errors(nms, ctx):
+    import torch
+    wl = ni.make_config("C2")                                      # Cartesian detector: no rings
+    _upload(nms, ctx, wl)
+    maps = torch.empty((1, wl.grid.n_q), dtype=torch.float32, device="cuda")
+    out = torch.empty((1, 2, 3), dtype=torch.float32, device="cuda")
+    with pytest.raises(nms.NmsError) as e:
+        nms.nms_modal_decomposition(ctx, maps, 1, 2, None, None, out, None)
+    assert e.value.status == nms.NMS_E_STATE                       # no grid yet
+    nms.nms_compute(ctx, wl.grid, [0], maps)
+    with pytest.raises(nms.NmsError) as e:
+        nms.nms_modal_decomposition(ctx, maps, 1, 2, None, None, out, None)
+    assert e.value.status == nms.NMS_E_UNSUPPORTED
+    wl = ni.make_config("C1")
+    _upload(nms, ctx, wl)
+    maps = torch.empty((1, wl.grid.n_q), dtype=torch.float32, device="cuda")
+    nms.nms_compute(ctx, wl.grid, [0], maps)
+    for bad in (-1, 64):
+        with pytest.raises(nms.NmsError) as e:
+            nms.nms_modal_decomposition(ctx, maps, 1, bad, None, None, out, None)
+        assert e.value.status == nms.NMS_E_ARG
+    with pytest.raises(nms.NmsError) as e:
+        nms.nms_modal_decomposition(ctx, maps, 1, 2, None, None, None, None)
+    assert e.value.status == nms.NMS_E_ARG
+
+
 def test_histogram_on_polar_grid_and_empty_bins(nms, ctx, oracle_mod):
     import torch
     wl = ni.make_config("C1")
