@@ -160,6 +160,18 @@ def azimuthal_hist(maps, qy, qz, n_bins: int, q_lo: float, q_hi: float):
     return out, cnt
 
 
+def correlation_2d(fmap, q, theta, rho, alpha):
+    """(Re C, Im C) [len(rho), len(alpha)] of Eq. 36 for one map [len(q) * len(theta)] on a polar grid."""
+    q, theta, rho, alpha = _f64(q), _f64(theta), _f64(rho), _f64(alpha)
+    fmap = _f64(fmap).reshape(q.shape[0] * theta.shape[0])
+    re, im = np.empty((rho.shape[0], alpha.shape[0])), np.empty((rho.shape[0], alpha.shape[0]))
+    _chk(lib().nmso_correlation_2d(_p(fmap, C.c_double), C.c_int(q.shape[0]), C.c_int(theta.shape[0]), _p(q, C.c_double),
+                                   _p(theta, C.c_double), C.c_int(rho.shape[0]), C.c_int(alpha.shape[0]),
+                                   _p(rho, C.c_double), _p(alpha, C.c_double), _p(re, C.c_double), _p(im, C.c_double)),
+         "correlation_2d")
+    return re, im
+
+
 def correlation(Iq, q, r, count=None):
     """(c, p) [n_maps, n_r] by the literal Eq. 34-35 trapezoid over the non-empty bins."""
     q, r = _f64(q), _f64(r)

@@ -21,7 +21,9 @@
  * values, sphere form factor, azimuthal means Eq. 65-67, Fourier-Bessel
  * of the sphere form factor (gamma_0), form/interference split of two
  * identical particles, angular modal decomposition of trigonometric maps
- * (A_0^c / A_2^c = -1 for sin^2, A_0^c / A_4^c = -1 for sin^2 cos^2, L199).
+ * (A_0^c / A_2^c = -1 for sin^2, A_0^c / A_4^c = -1 for sin^2 cos^2, L199),
+ * 2-D correlation of a ring (2 pi J0, -2 pi J2 cos 2 alpha), of a Gaussian,
+ * parity symmetries and brute force.
  * No function here is "parity unpinned".
  *
  * Build: gcc -O2 -fopenmp -shared -fPIC -o libnmso.so nmso.c -lm
@@ -397,6 +399,43 @@ int nmso_azimuthal_hist(const double *maps, int nm, const double *qy, const doub
             if (cnt[b] > 0) out_I[(int64_t)a * n_bins + b] /= (double)cnt[b];
     if (out_count) memcpy(out_count, cnt, sizeof(int32_t) * (size_t)n_bins);
     free(cnt);
+    return NMSO_OK;
+}
+
+/* ------------------------------------------------------------------------
+ * Two-dimensional correlation function, Eq. 36 (L213):
+ *   C(rho, alpha) = int_0^2pi int_0^inf f(q, theta) exp(i q rho cos(theta - alpha)) q dq dtheta,
+ * by the trapezoidal rule (L183) on the polar detector grid: periodic in theta (theta_j = 2 pi j / n1,
+ * weight 2 pi / n1, reading 7), non-uniform in q over the available abscissae only, no
+ * extrapolation to 0 or infinity (the reading taken for c(r), reading 9):
+ *   wq_0 = (q_1 - q_0)/2, wq_i = (q_{i+1} - q_{i-1})/2, wq_{n0-1} = (q_{n0-1} - q_{n0-2})/2  (n0 = 1: wq = 1).
+ * q cos(theta - alpha) rho = (q sin theta)(rho sin alpha) + (q cos theta)(rho cos alpha).
+ * map [n0][n1]; q [n0], theta [n1], rho [m0], alpha [m1] (float32 grid values promoted); out_re, out_im [m0][m1].
+ * ---------------------------------------------------------------------- */
+int nmso_correlation_2d(const double *map, int n0, int n1, const double *q, const double *theta,
+                        int m0, int m1, const double *rho, const double *alpha, double *out_re, double *out_im)
+{
+    if (!map || !q || !theta || !rho || !alpha || !out_re || !out_im || n0 <= 0 || n1 <= 0 || m0 <= 0 || m1 <= 0)
+        return NMSO_E_ARG;
+    const double dth = 2.0 * M_PI / (double)n1;
+#pragma omp parallel for schedule(static)
+    for (int64_t o = 0; o < (int64_t)m0 * m1; ++o) {
+        const int a = (int)(o / m1), b = (int)(o % m1);
+        const double ry = rho[a] * sin(alpha[b]), rz = rho[a] * cos(alpha[b]);
+        double re = 0.0, im = 0.0;
+        for (int i = 0; i < n0; ++i) {
+            double wq = 1.0;
+            if (n0 > 1) wq = i == 0 ? 0.5 * (q[1] - q[0]) : (i == n0 - 1 ? 0.5 * (q[n0 - 1] - q[n0 - 2]) : 0.5 * (q[i + 1] - q[i - 1]));
+            for (int j = 0; j < n1; ++j) {
+                const double w = map[(int64_t)i * n1 + j] * q[i] * wq * dth;
+                const double ph = (q[i] * sin(theta[j])) * ry + (q[i] * cos(theta[j])) * rz;
+                re += w * cos(ph);
+                im += w * sin(ph);
+            }
+        }
+        out_re[o] = re;
+        out_im[o] = im;
+    }
     return NMSO_OK;
 }
 

@@ -620,3 +620,70 @@ def test_modal_uniform_sphere_magnetic_channel(oracle_mod):
     Is, Ic, a_s, a_c, A_s, A_c = oracle_mod.modal(M, wl.grid.n0, wl.grid.n1, wl.grid.u1, 4)
     assert A_c[0, 0] / A_c[0, 2] == pytest.approx(-1.0, abs=0.02)
     assert np.abs(A_s[0]).max() < 1e-6
+
+
+# ----------------------------------------------------------------------------------------------------
+# two-dimensional correlation function, Eq. 36 (L213)
+# ----------------------------------------------------------------------------------------------------
+def test_correlation_2d_of_a_ring_is_bessel(oracle_mod):
+    """A single detector ring (n_q = 1, weight 1): the theta integral of exp(i x cos(theta - alpha)) is 2 pi J0(x) and
+    that of cos(2 theta) exp(i x cos(theta - alpha)) is 2 pi i^2 J2(x) cos 2 alpha (Jacobi-Anger); the periodic
+    trapezoid is exact to rounding for n_theta well above x.  scipy supplies J0, J2 (library routine, independent)."""
+    from scipy.special import jv
+    n1, q0 = 96, 0.8
+    th = _theta(n1)
+    rho = np.linspace(0.0, 20.0, 33).astype(np.float32).astype(np.float64)
+    al = _theta(12)
+    re, im = oracle_mod.correlation_2d(np.ones(n1), [q0], th, rho, al)
+    want = 2 * np.pi * q0 * jv(0, q0 * rho)                           # f q wq dtheta sum = q0 * 2 pi J0
+    np.testing.assert_allclose(re, np.repeat(want[:, None], 12, axis=1), atol=1e-6)
+    assert np.abs(im).max() < 1e-6
+    re2, im2 = oracle_mod.correlation_2d(np.cos(2 * th), [q0], th, rho, al)
+    want2 = -2 * np.pi * q0 * jv(2, q0 * rho)[:, None] * np.cos(2 * al)[None, :]
+    np.testing.assert_allclose(re2, want2, atol=2e-6)
+    assert np.abs(im2).max() < 2e-6
+    # an odd harmonic gives a purely imaginary C: int sin(theta) e^{i x cos(theta - alpha)} = 2 pi i J1(x) sin alpha
+    re3, im3 = oracle_mod.correlation_2d(np.sin(th), [q0], th, rho, al)
+    np.testing.assert_allclose(im3, 2 * np.pi * q0 * jv(1, q0 * rho)[:, None] * np.sin(al)[None, :], atol=2e-6)
+    assert np.abs(re3).max() < 2e-6
+
+
+def test_correlation_2d_of_a_gaussian(oracle_mod):
+    """f = exp(-q^2 s^2 / 2): C(rho) = 2 pi int f J0(q rho) q dq = (2 pi / s^2) exp(-rho^2 / (2 s^2)) (Hankel pair);
+    fine, long q grid (q_max s = 8); the trapezoid in q leaves the Euler-Maclaurin end term 2 pi h^2 / 12 (f q)'(0)
+    = 1.3e-5 for h = 0.005, a constant offset, which bounds the agreement."""
+    s_ = 2.0
+    q = np.linspace(0.0, 4.0, 801)
+    th = _theta(64)
+    f = np.repeat(np.exp(-0.5 * (q * s_) ** 2)[:, None], 64, axis=1)
+    rho = np.linspace(0.0, 6.0, 13)
+    re, im = oracle_mod.correlation_2d(f, q, th, rho, [0.0, 1.0])
+    want = 2 * np.pi / s_ ** 2 * np.exp(-0.5 * (rho / s_) ** 2)
+    np.testing.assert_allclose(re[:, 0], want, rtol=0, atol=2e-5)
+    np.testing.assert_allclose(re[:, 1], want, rtol=0, atol=2e-5)
+    assert re[0, 0] - want[0] == pytest.approx(-2 * np.pi * 0.005 ** 2 / 12, rel=0.05)     # the end term itself, at rho = 0
+    assert np.abs(im).max() < 1e-7          # theta_j are float32 values: the inversion symmetry holds to 2^-24
+
+
+def test_correlation_2d_brute_force_and_trapezoid_weights(oracle_mod):
+    """Literal Python loops with the non-uniform trapezoid weights written out by hand, on a random map."""
+    rng = np.random.Generator(np.random.Philox(36))
+    q = np.array([0.1, 0.25, 0.7, 1.0]); wq = np.array([0.075, 0.3, 0.375, 0.15])
+    n1 = 7
+    th = _theta(n1)
+    f = rng.normal(size=(4, n1))
+    rho, al = np.array([0.0, 1.5, 4.0]), np.array([0.3, 2.0])
+    re, im = oracle_mod.correlation_2d(f, q, th, rho, al)
+    for a in range(3):
+        for b in range(2):
+            z = 0j
+            for i in range(4):
+                for j in range(n1):
+                    z += f[i, j] * q[i] * wq[i] * (2 * math.pi / n1) * cmath.exp(1j * q[i] * rho[a] * math.cos(th[j] - al[b]))
+            assert re[a, b] == pytest.approx(z.real, rel=1e-12, abs=1e-14)
+            assert im[a, b] == pytest.approx(z.imag, rel=1e-12, abs=1e-14)
+    # C(0) is the plain integral of f q; C(rho, alpha + pi) = conj C(rho, alpha) for a real map
+    assert re[0, 0] == pytest.approx(float(((f * (q * wq)[:, None]).sum()) * 2 * math.pi / n1), rel=1e-12)
+    re2, im2 = oracle_mod.correlation_2d(f, q, th, rho, al + math.pi)
+    np.testing.assert_allclose(re2, re, atol=1e-12)
+    np.testing.assert_allclose(im2, -im, atol=1e-12)
