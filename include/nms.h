@@ -93,7 +93,8 @@ typedef enum {
     NMS_T_AZIMUTHAL = 3,    /* a-4                                                  */
     NMS_T_CORRELATION = 4,  /* a-5                                                  */
     NMS_T_MODAL = 5,        /* f-2 angular modal decomposition                      */
-    NMS_T_COUNT = 6
+    NMS_T_CORR2D = 6,       /* f-1 two-dimensional correlation function (its amplitude kernel) */
+    NMS_T_COUNT = 7
 } nms_timer;
 
 /* ---- context ---------------------------------------------------------------------------------- */
@@ -179,6 +180,19 @@ NMS_API nms_status nms_modal_decomposition(nms_ctx* ctx, const float* maps, int 
  * in fp64.  r [dev][n_r] (float); out_c, out_p [dev][n_maps][n_r] (float).                       */
 NMS_API nms_status nms_correlation(nms_ctx* ctx, const float* I, const float* q_of_bin, const int32_t* count,
                            int n_maps, int n_bins, const float* r, int n_r, float* out_c, float* out_p);
+
+/* ---- two-dimensional correlation function (f-1, Eq. 36) -------------------------------------- */
+
+/* C(rho, alpha) = int int f(q, theta) exp(i q rho cos(theta - alpha)) q dq dtheta of ONE map [dev][n_q] (float) given
+ * on the context's current grid, which must be polar (NMS_E_UNSUPPORTED otherwise), evaluated on the polar grid
+ * rgrid (type 0: u0 = rho [n0], u1 = alpha [n1] radians, host arrays).  Trapezoidal rule (L183): periodic in theta
+ * (weight 2 pi / n1, reading 7), non-uniform in q over the given abscissae without extrapolation (as reading 9):
+ * wq_0 = (q_1 - q_0)/2, wq_i = (q_{i+1} - q_{i-1})/2, wq_last = (q_last - q_{last-1})/2 (a single ring: wq = 1).
+ * It is the direct Fourier sum of a-2 with the roles exchanged -- the n_q detector pixels are the "cells"
+ * (position (q sin theta, q cos theta) in fp64, weight f q wq dtheta rounded once to fp32) and the (rho, alpha) points
+ * are the "detector" -- and runs the same amplitude kernels.  out_re, out_im [dev][n0*n1] (float; either may be
+ * NULL).  The context's sample, detector grid and stored amplitudes are left untouched.                       */
+NMS_API nms_status nms_correlation_2d(nms_ctx* ctx, const float* map, const nms_qgrid* rgrid, float* out_re, float* out_im);
 
 /* ---- form factor / interference split (a-6, Eq. 49-50) -------------------------------- */
 

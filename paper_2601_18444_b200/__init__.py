@@ -26,7 +26,7 @@ LIB_PATH = os.path.join(_HERE, "libnms.so")
 
 KINDS = ["NUC", "MAG", "UNPOL", "PROJ", "NM", "SF", "CHI", "PM", "MP", "PP", "MM", "POL_PLUS", "POL_MINUS"]
 NMS_OK, NMS_E_ARG, NMS_E_STATE, NMS_E_CUDA, NMS_E_NOMEM, NMS_E_UNSUPPORTED = range(6)
-NMS_T_PREP, NMS_T_AMPLITUDE, NMS_T_EPILOGUE, NMS_T_AZIMUTHAL, NMS_T_CORRELATION, NMS_T_MODAL = range(6)
+NMS_T_PREP, NMS_T_AMPLITUDE, NMS_T_EPILOGUE, NMS_T_AZIMUTHAL, NMS_T_CORRELATION, NMS_T_MODAL, NMS_T_CORR2D = range(7)
 _STATUS = {0: "NMS_OK", 1: "NMS_E_ARG", 2: "NMS_E_STATE", 3: "NMS_E_CUDA", 4: "NMS_E_NOMEM", 5: "NMS_E_UNSUPPORTED"}
 
 EXPORTS = [
@@ -34,6 +34,7 @@ EXPORTS = [
     "nms_set_rotation", "nms_set_polarization", "nms_set_scales", "nms_amplitudes", "nms_response", "nms_compute",
     "nms_azimuthal_average", "nms_correlation", "nms_form_factor_split", "nms_run_host", "nms_get_weight_sums",
     "nms_set_option", "nms_get_info", "nms_kernel_time_ms", "nms_kernel_time_total", "nms_modal_decomposition",
+    "nms_correlation_2d",
 ]
 
 
@@ -185,6 +186,11 @@ def nms_azimuthal_average(ctx, maps, n_maps, n_bins, q_lo, q_hi, out_I, out_q=No
 def nms_modal_decomposition(ctx, maps, n_maps, k_max, out_Is=None, out_Ic=None, out_a=None, out_A=None):
     _check(ctx, _lib.nms_modal_decomposition(ctx, _dev(maps), C.c_int(n_maps), C.c_int(k_max), _dev(out_Is), _dev(out_Ic),
                                              _dev(out_a), _dev(out_A)))
+
+
+def nms_correlation_2d(ctx, fmap, rgrid, out_re=None, out_im=None):
+    g, keep = _grid_struct(rgrid)
+    _check(ctx, _lib.nms_correlation_2d(ctx, _dev(fmap), C.byref(g), _dev(out_re), _dev(out_im)))
 
 
 def nms_correlation(ctx, I, q_of_bin, count, n_maps, n_bins, r, out_c, out_p):

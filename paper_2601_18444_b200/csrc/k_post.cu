@@ -1,6 +1,7 @@
 // k_post.cu -- a-4 azimuthal average (Eq. 30, trapezoidal rule L183) and a-5 correlation function
 // c(r), p(r) (Eq. 34-35).  Both passes move at most a few MB: they are bounded by HBM traffic
 // in principle and by launch latency in practice.
+#include <utility>
 #include "nms_internal.h"
 
 namespace nms {
@@ -216,6 +217,109 @@ nms_status launch_azimuthal(nms_ctx* c, const float* maps, int n_maps, int n_bin
         c->launches += 3;
     }
     timer_end(c, NMS_T_AZIMUTHAL);
+    NMS_CUDA(c, cudaGetLastError());
+    return NMS_OK;
+}
+
+// ---- two-dimensional correlation function (Eq. 36) -----------------------------
+// C(rho, alpha) = sum_pixels w_p exp(+i (Y_p rho_y + Z_p rho_z)),  (Y_p, Z_p) = (q sin th, q cos th),
+// w_p = f_p q wq dtheta: the direct Fourier sum of k_amplitude.cu with the detector pixels as cells and the
+// (rho, alpha) points as detector.  Pass 1 writes the pixels as Cell records (weight in the nuclear channel);
+// the amplitude kernel then runs unchanged on them; pass 3 sums the chunk partials: C = conj(N~).
+__global__ void __launch_bounds__(256) k_pixel_cells(const float* __restrict__ map, const double2* __restrict__ qc,
+                                                     const float* __restrict__ u0, int n0, int n1,
+                                                     Cell* __restrict__ cells, TileMeta* __restrict__ meta)
+{
+    const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t n = (int64_t)n0 * n1;
+    if (p < n) {
+        const int i = (int)(p / n1);
+        const double q = (double)u0[i];
+        double wq = 1.0;                                   // non-uniform trapezoid in q, no extrapolation
+        if (n0 > 1)
+            wq = i == 0 ? 0.5 * ((double)u0[1] - q)
+                        : (i == n0 - 1 ? 0.5 * (q - (double)u0[n0 - 2]) : 0.5 * ((double)u0[i + 1] - (double)u0[i - 1]));
+        const double2 yz = qc[p];                           // (q sin th, q cos th) in fp64 (k_qsetup)
+        Cell ce;
+        ce.Y = yz.x; ce.Z = yz.y;
+        ce.wN = (float)((double)map[p] * q * wq * (6.283185307179586476925 / (double)n1));
+        ce.wx = 0.f; ce.wy = 0.f; ce.wz = 0.f;
+        cells[p] = ce;
+    }
+    if (p % TILE == 0 && p < n) {
+        TileMeta tm;
+        tm.Y0 = 0.0; tm.Z0 = 0.0; tm.first_slot = p; tm.n_slots = (int32_t)((n - p) < TILE ? (n - p) : TILE);
+        tm.flags = 3; tm.ext = 0.f; tm.pad_ = 0;
+        meta[p / TILE] = tm;
+    }
+}
+
+__global__ void __launch_bounds__(256) k_corr2d_finish(const double* __restrict__ part, int n_chunks, int64_t n_r,
+                                                       float* __restrict__ out_re, float* __restrict__ out_im)
+{
+    const int64_t f = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (f >= n_r) return;
+    double re = 0.0, im = 0.0;
+    for (int ch = 0; ch < n_chunks; ++ch) {
+        re += part[((int64_t)ch * 8 + 0) * n_r + f];
+        im += part[((int64_t)ch * 8 + 1) * n_r + f];
+    }
+    if (out_re) out_re[f] = (float)re;
+    if (out_im) out_im[f] = (float)(-im);      // the kernel sums exp(-i Psi): C = conj
+}
+
+nms_status launch_correlation_2d(nms_ctx* c, const float* map, const nms_qgrid* rgrid, float* out_re, float* out_im)
+{
+    const int64_t n_pix = c->n_q;
+    const int64_t n_tiles = (n_pix + TILE - 1) / TILE;
+    if (nms_status st = ensure(c, c->pix_cells, sizeof(Cell) * (size_t)n_pix)) return st;
+    if (nms_status st = ensure(c, c->pix_meta, sizeof(TileMeta) * (size_t)n_tiles)) return st;
+    k_pixel_cells<<<(unsigned)((n_pix + 255) / 256), 256, 0, c->stream>>>(map, (const double2*)c->qc.p, (const float*)c->u0.p,
+                                                                          c->g_n0, c->g_n1, (Cell*)c->pix_cells.p,
+                                                                          (TileMeta*)c->pix_meta.p);
+    c->launches += 1;
+    NMS_CUDA(c, cudaGetLastError());
+
+    // run the amplitude path on (pixels, r-grid): exchange the context's sample and grid state, restore afterwards
+    struct Saved {
+        DevBuf cells, tile_meta, u0, u1, qc, sc;
+        int64_t n_tiles, n_slots, W, K, n_q;
+        bool grid_valid, g_uniform, has_N, has_M;
+        int g_type, g_n0, g_n1;
+        double g_dq;
+        std::vector<float> h_u0, h_u1;
+    } sv;
+    auto exchange = [&]() {
+        std::swap(sv.cells, c->cells); std::swap(sv.tile_meta, c->tile_meta);
+        std::swap(sv.u0, c->u0); std::swap(sv.u1, c->u1); std::swap(sv.qc, c->qc); std::swap(sv.sc, c->sc);
+        std::swap(sv.n_tiles, c->n_tiles); std::swap(sv.n_slots, c->n_slots); std::swap(sv.W, c->W); std::swap(sv.K, c->K);
+        std::swap(sv.n_q, c->n_q); std::swap(sv.grid_valid, c->grid_valid); std::swap(sv.g_uniform, c->g_uniform);
+        std::swap(sv.has_N, c->has_N); std::swap(sv.has_M, c->has_M);
+        std::swap(sv.g_type, c->g_type); std::swap(sv.g_n0, c->g_n0); std::swap(sv.g_n1, c->g_n1); std::swap(sv.g_dq, c->g_dq);
+        std::swap(sv.h_u0, c->h_u0); std::swap(sv.h_u1, c->h_u1);
+    };
+    sv.cells = c->pix_cells; sv.tile_meta = c->pix_meta; sv.u0 = c->pix_u0; sv.u1 = c->pix_u1; sv.qc = c->pix_qc; sv.sc = c->pix_sc;
+    sv.n_tiles = n_tiles; sv.n_slots = n_pix; sv.W = n_pix; sv.K = 0; sv.n_q = 0;
+    sv.grid_valid = false; sv.g_uniform = false; sv.has_N = true; sv.has_M = false;
+    sv.g_type = 0; sv.g_n0 = 0; sv.g_n1 = 0; sv.g_dq = 0.0;
+    exchange();                                   // the context now describes the pixel sample, no grid yet
+    nms_status st = set_grid(c, rgrid);
+    AmpPlan plan;
+    if (!st) st = plan_amplitude(c, false, &plan);
+    if (!st) {
+        timer_begin(c, NMS_T_CORR2D);
+        st = launch_amplitude(c, plan, nullptr, 0);
+        if (!st) {
+            const int64_t n_r = c->n_q;
+            k_corr2d_finish<<<(unsigned)((n_r + 255) / 256), 256, 0, c->stream>>>((const double*)c->part.p, c->n_chunks_used,
+                                                                                   n_r, out_re, out_im);
+            c->launches += 1;
+        }
+        timer_end(c, NMS_T_CORR2D);
+    }
+    exchange();                                   // back: sv holds the pixel / r-grid buffers again (possibly regrown)
+    c->pix_cells = sv.cells; c->pix_meta = sv.tile_meta; c->pix_u0 = sv.u0; c->pix_u1 = sv.u1; c->pix_qc = sv.qc; c->pix_sc = sv.sc;
+    if (st) return st;
     NMS_CUDA(c, cudaGetLastError());
     return NMS_OK;
 }

@@ -151,7 +151,7 @@ static nms_status set_sample_impl(nms_ctx* c, const float* pos, const float* N, 
     return repack(c);
 }
 
-static nms_status set_grid(nms_ctx* c, const nms_qgrid* g)
+nms_status set_grid(nms_ctx* c, const nms_qgrid* g)
 {
     if (!g) return fail(c, NMS_E_ARG, "grid is NULL");
     if (g->type < 0 || g->type > 2) return fail(c, NMS_E_ARG, "grid type %d unknown", g->type);
@@ -245,7 +245,8 @@ void nms_destroy(nms_ctx* c)
     cudaStreamSynchronize(c->stream);
     DevBuf* bufs[] = {&c->raw_pos, &c->raw_N, &c->raw_m, &c->centres, &c->tile_src, &c->tile_meta, &c->cells,
                       &c->wsum, &c->u0, &c->u1, &c->qc, &c->sc, &c->amp64, &c->part, &c->ppart, &c->formpart,
-                      &c->chunk_begin, &c->kinds_dev, &c->bin_idx, &c->bin_sum, &c->bin_cnt, &c->modal_tab, &c->modal_ring};
+                      &c->chunk_begin, &c->kinds_dev, &c->bin_idx, &c->bin_sum, &c->bin_cnt, &c->modal_tab, &c->modal_ring,
+                      &c->pix_cells, &c->pix_meta, &c->pix_u0, &c->pix_u1, &c->pix_qc, &c->pix_sc};
     for (DevBuf* b : bufs) free_buf(*b);
     for (DevBuf& b : c->host_stage) free_buf(b);
     for (Timer& t : c->timers) {
@@ -402,6 +403,17 @@ nms_status nms_modal_decomposition(nms_ctx* c, const float* maps, int n_maps, in
     if (k_max < 0 || k_max > 63) return fail(c, NMS_E_ARG, "k_max = %d outside 0..63", k_max);
     if (!out_Is && !out_Ic && !out_a && !out_A) return fail(c, NMS_E_ARG, "no output requested");
     return launch_modal(c, maps, n_maps, k_max, out_Is, out_Ic, out_a, out_A);
+}
+
+nms_status nms_correlation_2d(nms_ctx* c, const float* map, const nms_qgrid* rgrid, float* out_re, float* out_im)
+{
+    CHECK_CTX(c);
+    if (!c->grid_valid) return fail(c, NMS_E_STATE, "nms_correlation_2d needs a current grid (nms_amplitudes / nms_compute)");
+    if (c->g_type != 0) return fail(c, NMS_E_UNSUPPORTED, "nms_correlation_2d needs a polar detector grid");
+    if (!map || !rgrid || (!out_re && !out_im)) return fail(c, NMS_E_ARG, "NULL argument");
+    if (rgrid->type != 0 || rgrid->n0 <= 0 || rgrid->n1 <= 0 || !rgrid->u0 || !rgrid->u1)
+        return fail(c, NMS_E_ARG, "the (rho, alpha) grid must be polar with positive sizes");
+    return launch_correlation_2d(c, map, rgrid, out_re, out_im);
 }
 
 nms_status nms_correlation(nms_ctx* c, const float* I, const float* q_of_bin, const int32_t* count, int n_maps, int n_bins,

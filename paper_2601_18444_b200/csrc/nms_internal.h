@@ -102,6 +102,7 @@ struct nms_ctx {
     std::vector<int32_t> h_chunk_begin;
     nms::DevBuf kinds_dev;             // int32 [<=13]
     nms::DevBuf bin_idx, bin_sum, bin_cnt;
+    nms::DevBuf pix_cells, pix_meta, pix_u0, pix_u1, pix_qc, pix_sc;   // 2-D correlation: detector pixels as a sample, r-grid
     nms::DevBuf modal_tab, modal_ring; // (sin, cos)(k theta_j) table; fp64 ring values of the modal decomposition
     nms::DevBuf host_stage[8];         // device staging for nms_run_host
 
@@ -126,6 +127,8 @@ void timer_end(nms_ctx* c, int which);
 // k_prep.cu
 nms_status launch_prep(nms_ctx* c);                       // a-1: raw sample -> packed tiles, wsum
 nms_status launch_qsetup(nms_ctx* c);                     // detector abscissae -> qc, sc
+// nms_api.cu
+nms_status set_grid(nms_ctx* c, const nms_qgrid* g);      // install a detector grid as the current one
 // k_amplitude.cu
 struct AmpPlan {
     int variant;       // 1 list direct, 2 polar direct, 4 cartesian direct, 3 polar / 5 cartesian recurrence, 8 exact
@@ -148,6 +151,7 @@ nms_status launch_azimuthal(nms_ctx* c, const float* maps, int n_maps, int n_bin
                             float* out_I, float* out_q, int32_t* out_count);
 nms_status launch_modal(nms_ctx* c, const float* maps, int n_maps, int k_max, float* out_Is, float* out_Ic, float* out_a,
                         float* out_A);
+nms_status launch_correlation_2d(nms_ctx* c, const float* map, const nms_qgrid* rgrid, float* out_re, float* out_im);
 nms_status launch_correlation(nms_ctx* c, const float* I, const float* q_of_bin, const int32_t* count, int n_maps,
                               int n_bins, const float* r, int n_r, float* out_c, float* out_p);
 

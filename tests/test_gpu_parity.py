@@ -445,6 +445,77 @@ def test_modal_decomposition_errors(nms, ctx):
     assert e.value.status == nms.NMS_E_ARG
 
 
+@pytest.mark.parametrize("variant", [0, 1, 2])
+def test_correlation_2d(nms, ctx, oracle_mod, variant):
+    """f-1, Eq. 36: C(rho, alpha) of the GPU's own maps (pass-isolated) against the oracle; the criterion is the
+    north-star amplitude criterion of the underlying Fourier sum, |dC| <= 1e-5 sum_p |w_p| with w_p = f q wq dtheta.
+    The chiral-type odd map gives a purely imaginary C, the even ones a real C (checked on the oracle side)."""
+    import torch
+    wl = ni.make_config("C5", small=True)
+    kinds = [KI["UNPOL"], KI["SF"], KI["CHI"]]
+    _upload(nms, ctx, wl)
+    n0, n1 = wl.grid.n0, wl.grid.n1
+    maps = torch.empty((len(kinds), wl.grid.n_q), dtype=torch.float32, device="cuda")
+    nms.nms_compute(ctx, wl.grid, kinds, maps)
+    rgrid = ni.polar_grid(np.linspace(0.0, 30.0, 21 if variant != 2 else 24), 36)
+    re = torch.empty(rgrid.n_q, dtype=torch.float32, device="cuda")
+    im = torch.empty_like(re)
+    maps_h = maps.cpu().numpy()
+    q64 = wl.grid.u0.astype(np.float64)
+    wq = np.empty(n0)
+    wq[0], wq[-1] = 0.5 * (q64[1] - q64[0]), 0.5 * (q64[-1] - q64[-2])
+    wq[1:-1] = 0.5 * (q64[2:] - q64[:-2])
+    nms.nms_set_option(ctx, "variant", variant)
+    for i in range(len(kinds)):
+        nms.nms_correlation_2d(ctx, maps[i], rgrid, re, im)
+        nms.nms_synchronize(ctx)
+        if variant == 0:
+            assert nms.nms_get_info(ctx, "variant_used") == 8          # small problem: exact kernel
+        if variant == 2:
+            assert nms.nms_get_info(ctx, "variant_used") == 3          # rho is an arithmetic progression: recurrence
+        rre, rim = oracle_mod.correlation_2d(maps_h[i], wl.grid.u0, wl.grid.u1, rgrid.u0, rgrid.u1)
+        sw = float((np.abs(maps_h[i].astype(np.float64)).reshape(n0, n1) * (q64 * wq)[:, None]).sum() * 2 * np.pi / n1)
+        tol = (1e-5 if variant else 2e-7) * sw
+        assert np.abs(re.cpu().numpy().reshape(rgrid.n0, rgrid.n1) - rre).max() <= tol, ni.KINDS[kinds[i]]
+        assert np.abs(im.cpu().numpy().reshape(rgrid.n0, rgrid.n1) - rim).max() <= tol, ni.KINDS[kinds[i]]
+    nms.nms_set_option(ctx, "variant", 0)
+    # the detector grid, the sample and the stored amplitudes of the context are untouched
+    maps2 = torch.empty_like(maps)
+    nms.nms_compute(ctx, wl.grid, kinds, maps2)
+    nms.nms_synchronize(ctx)
+    assert torch.equal(maps, maps2)
+    I = torch.empty((len(kinds), n0), dtype=torch.float32, device="cuda")
+    nms.nms_azimuthal_average(ctx, maps, len(kinds), n0, 0.0, 0.0, I)
+    nms.nms_synchronize(ctx)
+    np.testing.assert_allclose(I.cpu().numpy(), oracle_mod.azimuthal_polar(maps_h, n0, n1), rtol=2e-6, atol=1e-6 * np.abs(maps_h).max())
+
+
+def test_correlation_2d_errors(nms, ctx):
+    import torch
+    wl = ni.make_config("C2")
+    _upload(nms, ctx, wl)
+    maps = torch.empty((1, wl.grid.n_q), dtype=torch.float32, device="cuda")
+    out = torch.empty(8, dtype=torch.float32, device="cuda")
+    rgrid = ni.polar_grid(np.linspace(0.0, 1.0, 2), 4)
+    with pytest.raises(nms.NmsError) as e:
+        nms.nms_correlation_2d(ctx, maps[0], rgrid, out, None)
+    assert e.value.status == nms.NMS_E_STATE
+    nms.nms_compute(ctx, wl.grid, [0], maps)
+    with pytest.raises(nms.NmsError) as e:
+        nms.nms_correlation_2d(ctx, maps[0], rgrid, out, None)
+    assert e.value.status == nms.NMS_E_UNSUPPORTED                  # Cartesian detector
+    wl = ni.make_config("C1")
+    _upload(nms, ctx, wl)
+    maps = torch.empty((1, wl.grid.n_q), dtype=torch.float32, device="cuda")
+    nms.nms_compute(ctx, wl.grid, [0], maps)
+    with pytest.raises(nms.NmsError) as e:
+        nms.nms_correlation_2d(ctx, maps[0], ni.cartesian_grid(np.zeros(2), np.zeros(2)), out, None)
+    assert e.value.status == nms.NMS_E_ARG
+    with pytest.raises(nms.NmsError) as e:
+        nms.nms_correlation_2d(ctx, maps[0], rgrid, None, None)
+    assert e.value.status == nms.NMS_E_ARG
+
+
 def test_histogram_on_polar_grid_and_empty_bins(nms, ctx, oracle_mod):
     import torch
     wl = ni.make_config("C1")
