@@ -216,6 +216,32 @@ class Runner:
         self.ctx.close()
 
 
+def time_next_rows(nms, run, wl, torch, dev, reps=3):
+    """SURVEY 8(f) rows built so far, timed OUTSIDE the step on the step's last maps (polar detectors only):
+    f-2 angular modal decomposition of all maps (k_max = 8) and f-1 two-dimensional correlation function of the
+    first map on a (rho, alpha) grid of the detector's own size -- the amplitude kernel with pixels as cells."""
+    h, nk, g = run.h, len(wl.kinds), wl.grid
+    k_max = 8
+    f32 = dict(dtype=torch.float32, device=dev)
+    Is, Ic = torch.empty((nk, k_max + 1, g.n0), **f32), torch.empty((nk, k_max + 1, g.n0), **f32)
+    a, A = torch.empty((nk, 2, k_max + 1), **f32), torch.empty((nk, 2, k_max + 1), **f32)
+    r_max = float(np.pi / max(float(g.u0[1] - g.u0[0]), 1e-30)) if g.n0 > 1 else 1.0      # Nyquist range of the q grid
+    rgrid = ni.polar_grid(np.linspace(0.0, r_max, g.n0), g.n1)
+    re, im = torch.empty(rgrid.n_q, **f32), torch.empty(rgrid.n_q, **f32)
+    out = {}
+    for name, fn, units in (("modal_f2", lambda: nms.nms_modal_decomposition(h, run.maps, nk, k_max, Is, Ic, a, A),
+                             nk * g.n_q * (k_max + 1)),
+                            ("correlation_2d_f1", lambda: nms.nms_correlation_2d(h, run.maps[0], rgrid, re, im),
+                             g.n_q * rgrid.n_q)):
+        fn()
+        ms = _timed(torch, dev, fn, reps) / reps
+        out[name] = {"ms": ms, "units": units, "gunits_per_s": units / (ms * 1e-3) / 1e9}
+    out["modal_f2"]["unit"] = "map values x harmonics"
+    out["correlation_2d_f1"]["unit"] = "pixel x r-point pairs (one complex amplitude)"
+    out["correlation_2d_f1"]["r_grid"] = f"polar {rgrid.n0}x{rgrid.n1}, rho <= {r_max:.1f}"
+    return out
+
+
 def _timed(torch, dev, fn, steps, dist=None):
     """Time exactly `steps` calls of fn between barrier + synchronize on both sides; ms, max over ranks."""
     if dist is not None:
@@ -425,6 +451,7 @@ def run_cuda(args, rank, local_rank, world):
     h2d, d2h = run.bytes_per_step()
     e2e = {"value": aggregate_rate(wl.pairs, world, ms_e2e), "unit": "Gpair/s", "ms_per_step": ms_e2e,
            "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": e2e_steps}
+    next_rows = time_next_rows(nms, run, wl, torch, dev) if wl.grid.type == 0 else None
     run.close()
 
     cpu_baseline = None
@@ -437,7 +464,7 @@ def run_cuda(args, rank, local_rank, world):
                 "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                 "config": workload_config(wl, {"parallelism": "replicas only" if world > 1 else "single GPU"}),
                 "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "passes": passes,
-                "cpu_baseline": cpu_baseline}
+                "next_rows": next_rows, "cpu_baseline": cpu_baseline}
         print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()

@@ -151,14 +151,19 @@ __device__ __forceinline__ u64 phasor(double m)
     return pack2(__cosf(x), __sinf(x));
 }
 
-// 4 packed accumulations of one (cell, detector point): acc[c] += {w_c, w_c} * {cos, sin}.  The pack of a
+// NCH packed accumulations of one (cell, detector point): acc[c] += {w_c, w_c} * {cos, sin}.  The pack of a
 // register with itself compiles to the broadcast operand form (FFMA2 Rd, Rw.F32, Rph, Racc): no extra move.
-__device__ __forceinline__ void accumulate(u64 (&acc)[4], const float4& w, u64 ph)
+// NCH = 4: nuclear + three magnetic channels; NCH = 1: nuclear only (sample without moments -- the activation
+// switch of L242 -- and the pixel sums of the two-dimensional correlation function).
+template <int NCH>
+__device__ __forceinline__ void accumulate(u64 (&acc)[NCH], const float4& w, u64 ph)
 {
     acc[0] = ffma2(pack2(w.x, w.x), ph, acc[0]);
-    acc[1] = ffma2(pack2(w.y, w.y), ph, acc[1]);
-    acc[2] = ffma2(pack2(w.z, w.z), ph, acc[2]);
-    acc[3] = ffma2(pack2(w.w, w.w), ph, acc[3]);
+    if (NCH > 1) {
+        acc[1 % NCH] = ffma2(pack2(w.y, w.y), ph, acc[1 % NCH]);
+        acc[2 % NCH] = ffma2(pack2(w.z, w.z), ph, acc[2 % NCH]);
+        acc[3 % NCH] = ffma2(pack2(w.w, w.w), ph, acc[3 % NCH]);
+    }
 }
 
 // Advance the phase of the phasor {c, s} by the step whose phasor is (cd, sd): {c cd - s sd, s cd + c sd}.
@@ -270,7 +275,7 @@ template <int QT, int NB> struct Seg {
 };
 
 // NB = 0: direct evaluation of every pair; NB > 0: line recurrence with NB exactly evaluated points per QT
-template <int MODE, int QT, bool SPLIT, int MINB, int NB>
+template <int MODE, int QT, bool SPLIT, int MINB, int NB, int NCH>
 __global__ void __launch_bounds__(AMP_THREADS, MINB) k_amp(const AmpArgs a)
 {
     static_assert(NB == 0 || (MODE != 2 && NB <= QT), "the recurrence needs a line of equally spaced abscissae");
@@ -336,7 +341,7 @@ __global__ void __launch_bounds__(AMP_THREADS, MINB) k_amp(const AmpArgs a)
         if (tile_beg + 1 < tile_end) issue_tile(a, tile_beg + 1, sC + STAGE_CELLS, &bar[1]);
     }
 
-    u64 acc[QT][4];            // per point and channel: {sum w cos, sum w sin}
+    u64 acc[QT][NCH];          // per point and channel: {sum w cos, sum w sin}
     bool first_total = true;   // SPLIT: no object of this chunk has been completed yet
 
     for (int t = tile_beg; t < tile_end; ++t) {
@@ -347,7 +352,7 @@ __global__ void __launch_bounds__(AMP_THREADS, MINB) k_amp(const AmpArgs a)
 #pragma unroll
         for (int k = 0; k < QT; ++k)
 #pragma unroll
-            for (int r = 0; r < 4; ++r) acc[k][r] = 0ull;
+            for (int r = 0; r < NCH; ++r) acc[k][r] = 0ull;
         mbar_wait(&bar[stage], (uint32_t)((it >> 1) & 1));
 
         const int nc = tm.n_slots;
@@ -369,7 +374,7 @@ __global__ void __launch_bounds__(AMP_THREADS, MINB) k_amp(const AmpArgs a)
                     ph[k] = phasor(m);
                 }
 #pragma unroll
-                for (int k = 0; k < QT; ++k) accumulate(acc[k], w, ph[k]);
+                for (int k = 0; k < QT; ++k) accumulate<NCH>(acc[k], w, ph[k]);
             } else {
                 // step phasor of this cell: phase step dq' p (polar) or dq' Z (Cartesian), exactly reduced
                 float cd, sd;
@@ -380,18 +385,18 @@ __global__ void __launch_bounds__(AMP_THREADS, MINB) k_amp(const AmpArgs a)
                     pb[b] = phasor(MODE == 0 ? fma(gb[b], p, MAGIC) : fma(gb[b], YZ.y, p) + MAGIC);
 #pragma unroll
                 for (int b = 0; b < NBX; ++b) {
-                    accumulate(acc[S::kb(b)], w, pb[b]);
+                    accumulate<NCH>(acc[S::kb(b)], w, pb[b]);
                     u64 ph = pb[b];
 #pragma unroll
                     for (int k = S::kb(b) + 1; k <= S::hi(b); ++k) {
                         ph = rotate(ph, cd, sd);
-                        accumulate(acc[k], w, ph);
+                        accumulate<NCH>(acc[k], w, ph);
                     }
                     ph = pb[b];
 #pragma unroll
                     for (int k = S::kb(b) - 1; k >= S::lo(b); --k) {
                         ph = rotate(ph, cd, -sd);
-                        accumulate(acc[k], w, ph);
+                        accumulate<NCH>(acc[k], w, ph);
                     }
                 }
             }
@@ -411,8 +416,8 @@ __global__ void __launch_bounds__(AMP_THREADS, MINB) k_amp(const AmpArgs a)
                 double Ap[8];
 #pragma unroll
                 for (int w = 0; w < 4; ++w) {
-                    float cs, sn;
-                    unpack2(acc[k][w], cs, sn);
+                    float cs = 0.f, sn = 0.f;
+                    if (w < NCH) unpack2(acc[k][w % NCH], cs, sn);
                     Ap[2 * w] = (double)cs;          // Re: + sum w cos(Psi)   (Eq. 44, 46)
                     Ap[2 * w + 1] = -(double)sn;     // Im: - sum w sin(Psi)   (Eq. 45, 47)
                 }
@@ -429,36 +434,38 @@ constexpr size_t AMP_SMEM = 2 * STAGE_CELLS * sizeof(Cell) + 2 * sizeof(uint64_t
 typedef void (*amp_kernel_t)(const AmpArgs);
 
 template <int MODE, int QT, int MINB, int NB>
-static amp_kernel_t pick_split(bool split)
+static amp_kernel_t pick_split(bool split, bool nuclear_only)
 {
-    return split ? (amp_kernel_t)k_amp<MODE, QT, true, MINB, NB> : (amp_kernel_t)k_amp<MODE, QT, false, MINB, NB>;
+    if (nuclear_only)
+        return split ? (amp_kernel_t)k_amp<MODE, QT, true, MINB, NB, 1> : (amp_kernel_t)k_amp<MODE, QT, false, MINB, NB, 1>;
+    return split ? (amp_kernel_t)k_amp<MODE, QT, true, MINB, NB, 4> : (amp_kernel_t)k_amp<MODE, QT, false, MINB, NB, 4>;
 }
 
 template <int MODE>
-static amp_kernel_t pick_rec(int nb, bool split)
+static amp_kernel_t pick_rec(int nb, bool split, bool nuc)
 {
     switch (nb) {
-    case 1: return pick_split<MODE, 8, 4, 1>(split);
-    case 3: return pick_split<MODE, 8, 4, 3>(split);
-    case 4: return pick_split<MODE, 8, 4, 4>(split);
-    default: return pick_split<MODE, 8, 4, 2>(split);
+    case 1: return pick_split<MODE, 8, 4, 1>(split, nuc);
+    case 3: return pick_split<MODE, 8, 4, 3>(split, nuc);
+    case 4: return pick_split<MODE, 8, 4, 4>(split, nuc);
+    default: return pick_split<MODE, 8, 4, 2>(split, nuc);
     }
 }
 
 // variant: 1 list direct, 2 polar direct, 4 cartesian direct, 3 polar recurrence, 5 cartesian recurrence
-// (all with fp32 accumulation over a tile), 8 exact (fp64)
-static amp_kernel_t pick_kernel(int variant, int qt, int nb, bool split)
+// (all with fp32 accumulation over a tile), 8 exact (fp64); nuc: the sample has no magnetic channel
+static amp_kernel_t pick_kernel(int variant, int qt, int nb, bool split, bool nuc)
 {
     switch (variant) {
-    case 1: return pick_split<2, 4, 4, 0>(split);
+    case 1: return pick_split<2, 4, 4, 0>(split, nuc);
     case 2:
-        if (qt == 4) return pick_split<0, 4, 4, 0>(split);
-        return pick_split<0, 8, 4, 0>(split);
+        if (qt == 4) return pick_split<0, 4, 4, 0>(split, nuc);
+        return pick_split<0, 8, 4, 0>(split, nuc);
     case 4:
-        if (qt == 4) return pick_split<1, 4, 4, 0>(split);
-        return pick_split<1, 8, 4, 0>(split);
-    case 3: return pick_rec<0>(nb, split);
-    case 5: return pick_rec<1>(nb, split);
+        if (qt == 4) return pick_split<1, 4, 4, 0>(split, nuc);
+        return pick_split<1, 8, 4, 0>(split, nuc);
+    case 3: return pick_rec<0>(nb, split, nuc);
+    case 5: return pick_rec<1>(nb, split, nuc);
     default: return split ? (amp_kernel_t)k_amp_f64<true> : (amp_kernel_t)k_amp_f64<false>;
     }
 }
@@ -501,7 +508,7 @@ nms_status plan_amplitude(nms_ctx* c, bool split, AmpPlan* plan)
         }
     }
     const size_t smem = variant == 8 ? 0 : AMP_SMEM;
-    amp_kernel_t kern = pick_kernel(variant, qt, c->opt_bases, split);
+    amp_kernel_t kern = pick_kernel(variant, qt, c->opt_bases, split, !c->has_M);
     NMS_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)AMP_SMEM));
     int occ = 0;
     NMS_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, AMP_THREADS, smem));
@@ -572,7 +579,7 @@ nms_status launch_amplitude(nms_ctx* c, const AmpPlan& plan, const int32_t* kind
     a.kinds = kinds_dev; a.n_kinds = n_kinds;
     a.rp.Px = c->P[0]; a.rp.Py = c->P[1]; a.rp.Pz = c->P[2]; a.rp.sN = c->sN; a.rp.sM = c->sM; a.rp.invV = c->invV;
 
-    amp_kernel_t kern = pick_kernel(plan.variant, plan.qt, c->opt_bases, plan.split);
+    amp_kernel_t kern = pick_kernel(plan.variant, plan.qt, c->opt_bases, plan.split, !c->has_M);
     NMS_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)AMP_SMEM));
     dim3 grid((unsigned)plan.n_qblocks, (unsigned)n_chunks);
     if (!plan.split)   // the kernel accumulates into its chunk partials with reductions

@@ -516,6 +516,33 @@ def test_correlation_2d_errors(nms, ctx):
     assert e.value.status == nms.NMS_E_ARG
 
 
+@pytest.mark.parametrize("which", ["nuclear_only", "magnetic_only"])
+@pytest.mark.parametrize("variant", [1, 2, 3])
+def test_activation_switches(nms, ctx, oracle_mod, which, variant):
+    """L242: a sample without moments (m NULL: the one-channel kernel instantiation) or without nuclear weights
+    (N NULL); the absent amplitudes must be exactly zero."""
+    import torch
+    wl = ni.make_config("C5", small=True)
+    N, m = (wl.N, None) if which == "nuclear_only" else (None, wl.m)
+    kinds = [KI["NUC"], KI["MAG"], KI["UNPOL"], KI["SF"]]
+    nms.nms_set_sample(ctx, _t(wl.pos), _t(N), _t(m), wl.R)
+    nms.nms_set_option(ctx, "variant", variant)
+    amp = torch.empty((8, wl.grid.n_q), dtype=torch.float32, device="cuda")
+    maps = torch.empty((len(kinds), wl.grid.n_q), dtype=torch.float32, device="cuda")
+    nms.nms_amplitudes(ctx, wl.grid, amp)
+    nms.nms_response(ctx, kinds, maps)
+    nms.nms_synchronize(ctx)
+    qy, qz, th = oracle_mod.grid_points(wl.grid)
+    A, wsum = oracle_mod.amplitudes(wl.pos, N, m, wl.R, qy, qz, return_wsum=True)
+    M = oracle_mod.response(A, th, kinds, P=wl.P)
+    assert_amplitudes(amp.cpu().numpy(), A, wsum, which)
+    got = maps.cpu().numpy()
+    live = [0, 2] if which == "nuclear_only" else [1, 2, 3]
+    assert_cross_sections(got[live], M[live], [kinds[i] for i in live], which)
+    dead = [i for i in range(len(kinds)) if i not in live]
+    assert np.all(got[dead] == 0.0)
+
+
 def test_histogram_on_polar_grid_and_empty_bins(nms, ctx, oracle_mod):
     import torch
     wl = ni.make_config("C1")
