@@ -40,6 +40,10 @@ import nms_inputs as ni  # noqa: E402  (seeded input generators only; no arithme
 
 FP32_LANE_INSTR_PER_PAIR = 12      # 8 accumulate FFMA + 4 for the phasor
 LANES_PER_SM = 128
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE k_amp launch from the committed ncu --set full captures
+# (profiles/r1c_amp_kernels.md); null for workloads that were not captured.  The kernel is ALU-bound: the figure
+# only documents that DRAM traffic is irrelevant (C5: 4.5e-4 B per pair).
+NCU_DRAM_BYTES_PER_LAUNCH = {"C5": 1.632596e9 + 0.365705e9, "C3": 4.167948e9 + 7.983503e9}
 
 
 def _env_int(name, default):
@@ -420,7 +424,8 @@ def run_cuda(args, rank, local_rank, world):
     peak = sm_count * LANES_PER_SM * peaks["sm_max_mhz"] * 1e6 / 1e12
     clocks = sampler.summary()
     roofline = {"bound": "alu", "kernel": "k_amp (a-2 amplitude sums)", "achieved": achieved, "peak": peak,
-                "unit": "T FP32 lane-instr/s (12 per pair)", "frac": achieved / peak, "traffic": None,
+                "unit": "T FP32 lane-instr/s (12 per pair)", "frac": achieved / peak,
+                "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(wl.name),
                 "peak_source": f"{sm_count} SMs x 128 FP32 lanes x sm_max_mhz {peaks['sm_max_mhz']:.0f} ({peak_src})",
                 "gpair_s_kernel": pairs_per_launch / (amp_ms_per_launch * 1e-3) / 1e9,
                 "ms_per_launch": amp_ms_per_launch, "launches_timed": amp_n,
