@@ -105,6 +105,16 @@ def response(amp, theta, kinds: Sequence[int], P=None, sN=1.0, sM=1.0, invV=1.0,
     return (out, Q) if return_Q else out
 
 
+def cross_spectra(amp, sM=1.0, invV=1.0):
+    """Fourier cross-correlation components of the magnetisation (Eq. 51-52), plain NumPy complex arithmetic:
+    G_ab = invV sM^2 M~_a M~_b^*, a, b in (x, y, z); returns (G^R, G^I) [9, n_q] with row 3 a + b.
+    amp [8, n_q] are the raw amplitude planes (Re N, Im N, Re Mx, Im Mx, ...); scales as in DESIGN.md reading 4."""
+    amp = _f64(amp)
+    M = [sM * (amp[2 + 2 * c] + 1j * amp[3 + 2 * c]) for c in range(3)]
+    G = np.stack([invV * M[a] * np.conj(M[b]) for a in range(3) for b in range(3)])
+    return np.ascontiguousarray(G.real), np.ascontiguousarray(G.imag)
+
+
 def form_factor_split(pos, N, m, offsets, kinds, qy, qz, theta, R=None, centres=None, P=None, sN=1.0, sM=1.0, invV=1.0):
     """(total, form) maps [n_kinds, n_q] (Eq. 49-50): total = B(sum A_p), form = sum B(A_p)."""
     pos, N, m = _f32(pos), _f32(N), _f32(m)

@@ -687,3 +687,52 @@ def test_correlation_2d_brute_force_and_trapezoid_weights(oracle_mod):
     re2, im2 = oracle_mod.correlation_2d(f, q, th, rho, al + math.pi)
     np.testing.assert_allclose(re2, re, atol=1e-12)
     np.testing.assert_allclose(im2, -im, atol=1e-12)
+
+
+# ----------------------------------------------------------------------------------------------------
+# Fourier cross-correlation components G_ab = M~_a M~_b^*, Eq. 51-52 (L397-L402)
+# ----------------------------------------------------------------------------------------------------
+def test_cross_spectra_reproduce_the_cross_sections(oracle_mod):
+    """The magnetic cross sections are contractions of G: with q^ = (0, s, c), |Q|^2 = |M~|^2 - |q^.M~|^2 gives
+    MAG = sum_ab (delta_ab - q^_a q^_b) G^R_ab (Eq. 4-5), and Eq. 14 gives CHI = 2 (P_y s + P_z c)(s G^I_zx - c G^I_yx);
+    both against the independently coded response routine, general P, scales and rotation; G is Hermitian."""
+    rng = np.random.Generator(np.random.Philox(51))
+    W = 40
+    pos = rng.uniform(-8, 8, size=(W, 3)).astype(np.float32)
+    N = rng.uniform(0.5, 1.5, size=W).astype(np.float32)
+    m = rng.normal(size=(W, 3)).astype(np.float32)
+    grid = ni.polar_grid(np.linspace(0.05, 2.0, 9), 16)
+    qy, qz, th = oracle_mod.grid_points(grid)
+    R = ni.rot_z(25.0) @ ni.rot_y(40.0)
+    P = np.array([0.3, -0.5, 0.8]); P /= np.linalg.norm(P)
+    sM, invV = 1.7, 0.01
+    A = oracle_mod.amplitudes(pos, N, m, R, qy, qz)
+    GR, GI = oracle_mod.cross_spectra(A, sM=sM, invV=invV)
+    MAG, CHI = oracle_mod.response(A, th, [KI["MAG"], KI["CHI"]], P=P, sM=sM, invV=invV)
+    qh = np.stack([np.zeros_like(th), np.sin(th), np.cos(th)])
+    mag = sum(((a == b) - qh[a] * qh[b]) * GR[3 * a + b] for a in range(3) for b in range(3))
+    np.testing.assert_allclose(mag, MAG, rtol=1e-11, atol=1e-12 * np.abs(MAG).max())
+    s, c = np.sin(th), np.cos(th)
+    chi = 2 * (P[1] * s + P[2] * c) * (s * GI[3 * 2 + 0] - c * GI[3 * 1 + 0])
+    np.testing.assert_allclose(chi, CHI, rtol=1e-10, atol=1e-12 * np.abs(MAG).max())
+    for a in range(3):
+        assert np.all(np.abs(GI[3 * a + a]) <= 1e-15 * GR[3 * a + a]) and np.all(GR[3 * a + a] >= 0.0)
+        for b in range(3):
+            np.testing.assert_allclose(GR[3 * a + b], GR[3 * b + a], rtol=1e-14, atol=1e-15 * np.abs(GR).max())
+            if a != b:
+                np.testing.assert_allclose(GI[3 * a + b], -GI[3 * b + a], rtol=1e-14, atol=1e-15 * np.abs(GR).max())
+
+
+def test_cross_spectra_uniform_magnetisation(oracle_mod):
+    """Uniform m = n: M~ = n F, so G_ab = n_a n_b |F|^2 is real (Eq. 51-52 with Eq. 60's M~), |F|^2 = NUC for N = 1."""
+    pos, N, m = ni.uniform_sphere_sample(radius=6.0, a=1.0, n=(0.6, 0.0, 0.8))
+    grid = ni.polar_grid(np.linspace(0.05, 1.5, 6), 12)
+    qy, qz, th = oracle_mod.grid_points(grid)
+    A = oracle_mod.amplitudes(pos, N, m, None, qy, qz)
+    GR, GI = oracle_mod.cross_spectra(A)
+    F2 = oracle_mod.response(A, th, [KI["NUC"]])[0]
+    n = np.array([0.6, 0.0, 0.8])
+    for a in range(3):
+        for b in range(3):
+            np.testing.assert_allclose(GR[3 * a + b], n[a] * n[b] * F2, rtol=1e-6, atol=1e-9 * F2.max())
+            assert np.abs(GI[3 * a + b]).max() <= 1e-9 * F2.max()
