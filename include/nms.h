@@ -142,6 +142,11 @@ NMS_API nms_status nms_amplitudes(nms_ctx* ctx, const nms_qgrid* grid, float* ou
 /* Response maps out [dev][n_kinds][n_q] (float) from the amplitudes of the last nms_amplitudes call
  * (NMS_E_STATE if there was none since the last sample change).                                  */
 NMS_API nms_status nms_response(nms_ctx* ctx, const nms_kind* kinds, int n_kinds, float* out);
+/* Fourier cross-correlation components of the magnetisation (f-4, Eq. 51-52) from the amplitudes of the
+ * last nms_amplitudes call (NMS_E_STATE if there was none since the last sample change):
+ *   G_ab = invV sM^2 M~_a M~_b^*,  a, b in (x, y, z),  out_GR = Re G, out_GI = Im G, each [dev][9][n_q] (float) with
+ * row 3 a + b; either may be NULL (not both).  G^R is symmetric, G^I antisymmetric.                      */
+NMS_API nms_status nms_cross_spectra(nms_ctx* ctx, float* out_GR, float* out_GI);
 /* Fused a-2 + a-3: amplitudes and all requested responses without materialising the amplitudes.
  * This is the call bench.py times.  out [dev][n_kinds][n_q] (float).                             */
 NMS_API nms_status nms_compute(nms_ctx* ctx, const nms_qgrid* grid, const nms_kind* kinds, int n_kinds, float* out);

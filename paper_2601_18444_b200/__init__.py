@@ -34,7 +34,7 @@ EXPORTS = [
     "nms_set_rotation", "nms_set_polarization", "nms_set_scales", "nms_amplitudes", "nms_response", "nms_compute",
     "nms_azimuthal_average", "nms_correlation", "nms_form_factor_split", "nms_run_host", "nms_get_weight_sums",
     "nms_set_option", "nms_get_info", "nms_kernel_time_ms", "nms_kernel_time_total", "nms_modal_decomposition",
-    "nms_correlation_2d",
+    "nms_correlation_2d", "nms_cross_spectra",
 ]
 
 
@@ -164,6 +164,10 @@ def nms_amplitudes(ctx, grid, out_amp=None):
 def nms_response(ctx, kinds, out):
     k, n = _kinds(kinds)
     _check(ctx, _lib.nms_response(ctx, k, C.c_int(n), _dev(out)))
+
+
+def nms_cross_spectra(ctx, out_GR=None, out_GI=None):
+    _check(ctx, _lib.nms_cross_spectra(ctx, _dev(out_GR), _dev(out_GI)))
 
 
 def nms_compute(ctx, grid, kinds, out):

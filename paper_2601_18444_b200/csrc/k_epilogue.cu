@@ -58,6 +58,40 @@ __global__ void __launch_bounds__(256) k_epilogue(const EpiArgs a)
     }
 }
 
+// Fourier cross-correlation components (Eq. 51-52): G_ab = invV sM^2 M~_a M~_b^*, a, b in (x, y, z),
+// from the stored fp64 amplitudes; rows 3 a + b of G^R and G^I.
+__global__ void __launch_bounds__(256) k_cross_spectra(const double* __restrict__ amp64, int64_t n_q, double scale,
+                                                       float* __restrict__ out_GR, float* __restrict__ out_GI)
+{
+    const int64_t f = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (f >= n_q) return;
+    double re[3], im[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        re[c] = amp64[(int64_t)(2 + 2 * c) * n_q + f];
+        im[c] = amp64[(int64_t)(3 + 2 * c) * n_q + f];
+    }
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+#pragma unroll
+        for (int b = 0; b < 3; ++b) {
+            // (ra + i ia)(rb - i ib) = (ra rb + ia ib) + i (ia rb - ra ib)
+            if (out_GR) out_GR[(int64_t)(3 * a + b) * n_q + f] = (float)(scale * (re[a] * re[b] + im[a] * im[b]));
+            if (out_GI) out_GI[(int64_t)(3 * a + b) * n_q + f] = (float)(scale * (im[a] * re[b] - re[a] * im[b]));
+        }
+}
+
+nms_status launch_cross_spectra(nms_ctx* c, float* out_GR, float* out_GI)
+{
+    const unsigned blocks = (unsigned)((c->n_q + 255) / 256);
+    timer_begin(c, NMS_T_EPILOGUE);
+    k_cross_spectra<<<blocks, 256, 0, c->stream>>>((const double*)c->amp64.p, c->n_q, c->invV * c->sM * c->sM, out_GR, out_GI);
+    timer_end(c, NMS_T_EPILOGUE);
+    c->launches += 1;
+    NMS_CUDA(c, cudaGetLastError());
+    return NMS_OK;
+}
+
 static void fill_rp(const nms_ctx* c, RespParams& rp)
 {
     rp.Px = c->P[0]; rp.Py = c->P[1]; rp.Pz = c->P[2];

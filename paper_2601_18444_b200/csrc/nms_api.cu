@@ -354,6 +354,14 @@ nms_status nms_response(nms_ctx* c, const nms_kind* kinds, int n_kinds, float* o
     return launch_response_from_amp(c, kd, n_kinds, out);
 }
 
+nms_status nms_cross_spectra(nms_ctx* c, float* out_GR, float* out_GI)
+{
+    CHECK_CTX(c);
+    if (!c->amp_valid) return fail(c, NMS_E_STATE, "nms_cross_spectra needs a preceding nms_amplitudes on the current sample");
+    if (!out_GR && !out_GI) return fail(c, NMS_E_ARG, "no output requested");
+    return launch_cross_spectra(c, out_GR, out_GI);
+}
+
 nms_status nms_compute(nms_ctx* c, const nms_qgrid* grid, const nms_kind* kinds, int n_kinds, float* out)
 {
     CHECK_CTX(c);

@@ -143,6 +143,7 @@ nms_status launch_amplitude(nms_ctx* c, const AmpPlan& plan, const int32_t* kind
 // k_epilogue.cu
 nms_status launch_epilogue(nms_ctx* c, int n_chunks, const int32_t* kinds_dev, int n_kinds, float* out_maps,
                            float* out_amp, bool keep_amp64);
+nms_status launch_cross_spectra(nms_ctx* c, float* out_GR, float* out_GI);
 nms_status launch_response_from_amp(nms_ctx* c, const int32_t* kinds_dev, int n_kinds, float* out_maps);
 nms_status launch_split_epilogue(nms_ctx* c, int n_chunks, const int32_t* kinds_dev, int n_kinds, float* out_total,
                                  float* out_form);

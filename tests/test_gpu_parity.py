@@ -543,6 +543,39 @@ def test_activation_switches(nms, ctx, oracle_mod, which, variant):
     assert np.all(got[dead] == 0.0)
 
 
+@pytest.mark.parametrize("name,small", [("C2", False), ("C5", True)])
+def test_cross_spectra(nms, ctx, oracle_mod, name, small):
+    """f-4, Eq. 51-52: G_ab = invV sM^2 M~_a M~_b^* from the stored amplitudes, with scales; each component within
+    1e-3 relative above 1e-6 of the largest |G| (the north-star cross-section criterion), exact kernel and MUFU kernel."""
+    import torch
+    wl = ni.make_config(name, small=small)
+    _upload(nms, ctx, wl)
+    sM, invV = 2.5, 1e-3
+    nms.nms_set_scales(ctx, 1.0, sM, invV)
+    qy, qz, th = oracle_mod.grid_points(wl.grid)
+    A = oracle_mod.amplitudes(wl.pos, wl.N, wl.m, wl.R, qy, qz)
+    rGR, rGI = oracle_mod.cross_spectra(A, sM=sM, invV=invV)
+    gmax = np.abs(rGR).max()
+    GR = torch.empty((9, wl.grid.n_q), dtype=torch.float32, device="cuda")
+    GI = torch.empty_like(GR)
+    with pytest.raises(nms.NmsError) as e:
+        nms.nms_cross_spectra(ctx, GR, GI)
+    assert e.value.status == nms.NMS_E_STATE                       # no amplitudes yet
+    for variant in (0, 1):
+        nms.nms_set_option(ctx, "variant", variant)
+        nms.nms_amplitudes(ctx, wl.grid, None)
+        nms.nms_cross_spectra(ctx, GR, GI)
+        nms.nms_synchronize(ctx)
+        floor = (1e-6 if variant == 0 else 1e-5) * gmax            # reading 16: off-diagonal components are signed
+        for got, ref in ((GR.cpu().numpy(), rGR), (GI.cpu().numpy(), rGI)):
+            sel = np.abs(ref) > floor
+            assert np.all(np.abs(got[sel] - ref[sel]) <= 1e-3 * np.abs(ref[sel]))
+            assert np.all(np.abs(got - ref) <= 1e-3 * np.abs(ref) + 1e-3 * floor)
+    with pytest.raises(nms.NmsError) as e:
+        nms.nms_cross_spectra(ctx, None, None)
+    assert e.value.status == nms.NMS_E_ARG
+
+
 def test_histogram_on_polar_grid_and_empty_bins(nms, ctx, oracle_mod):
     import torch
     wl = ni.make_config("C1")
