@@ -308,7 +308,7 @@ def oracle_sample(wl, n_sample):
     n = min(n_sample, wl.grid.n_q)
     if n == wl.grid.n_q:
         return np.arange(n, dtype=np.int64)
-    return ni.q_subset(wl.grid.n_q, n, 9000 + int(wl.name[1]))
+    return ni.q_subset(wl.grid.n_q, n, 9000 + (int(wl.name[1]) if wl.name[1].isdigit() else 0))
 
 
 def time_oracle(wl, target_s=12.0, steps=1, warmup=0):
@@ -362,6 +362,7 @@ WORKLOAD_TEXT = {
     "C3": "ensemble of 1000 spheres (R = 5 nm, 0.5 nm cells), total and form-factor outputs",
     "C4": "skyrmion-lattice film 512x512x8, rocking scan of 36 rotations about z",
     "C5": "micromagnetic block 256^3 with 5 % pores, all responses, I(q), c(r), p(r)",
+    "S4C": "context only: synthetic re-creation of the paper's Sec. IV C run (800 spheres x 4224 cells, 1000x1000 grid)",
 }
 
 
@@ -480,7 +481,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="C5", choices=["C1", "C2", "C3", "C4", "C5"])
+    ap.add_argument("--workload", default="C5", choices=["C1", "C2", "C3", "C4", "C5", "S4C"])
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--oracle-seconds", type=float, default=12.0, help="CPU seconds per oracle step (bounded sample)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
