@@ -17,9 +17,10 @@ evaluated (no symmetry or merging tricks).  Rank 0 prints ONE JSON line.
  * cpu_baseline the fp64 oracle as it stands, timed on this box's host cores on a bounded sample
  * --impl reference   the oracle alone (this tier's reference arm), same metric and config
 
-N > 1 (torchrun): the path runs on one GPU (north_star); every rank runs an independent replica of the
-workload on its own GPU ("replicas only"), no data-path collective; value = total
-pairs of all ranks / max-over-ranks time; scaling = weak.
+N > 1 (torchrun): the path runs on one GPU (north_star); by default every rank runs an independent replica of
+the workload on its own GPU, no data-path collective; value = total pairs of all ranks /
+max-over-ranks time; scaling = weak.  --shard lines splits the detector lines of ONE workload over the ranks
+(cells replicated, all-gather of I(q) only); scaling = strong.
 """
 from __future__ import annotations
 
@@ -119,9 +120,10 @@ class ClockSampler:
 class Runner:
     """Owns one context, the device-resident raw arrays of one workload and its output buffers."""
 
-    def __init__(self, nms, wl, device: int):
+    def __init__(self, nms, wl, device: int, shard=None):
         import torch
         self.nms, self.wl, self.torch = nms, wl, torch
+        self.shard = shard                       # None, or (full workload, world, rank, dist) under --shard lines
         self.dev = torch.device("cuda", device)
         self.ctx = nms.Context(device)
         self.h = self.ctx.h
@@ -158,8 +160,16 @@ class Runner:
         nms, wl, h = self.nms, self.wl, self.h
         if self.nb:
             nms.nms_azimuthal_average(h, self.maps, len(wl.kinds), self.nb, wl.q_lo, wl.q_hi, self.I, self.qb, self.cnt)
-            if self.nr:
+            if self.nr and self.shard is None:
                 nms.nms_correlation(h, self.I, self.qb, self.cnt, len(wl.kinds), self.nb, self.d_r, self.c, self.p)
+            elif self.nr:
+                full, world, rank, dist = self.shard                  # every ring is needed: all-gather I(q)
+                nms.nms_synchronize(h)
+                I_full = gather_lines(self.I, full.grid.n0, world, rank, dist)
+                if not hasattr(self, "q_full"):
+                    self.q_full = self.torch.as_tensor(full.grid.u0, device=self.dev)
+                    self.cnt_full = self.torch.full((full.grid.n0,), full.grid.n1, dtype=self.torch.int32, device=self.dev)
+                nms.nms_correlation(h, I_full, self.q_full, self.cnt_full, len(wl.kinds), full.grid.n0, self.d_r, self.c, self.p)
 
     def step_device(self, d2h: bool = False):
         nms, wl, h = self.nms, self.wl, self.h
@@ -188,7 +198,7 @@ class Runner:
     # -- the same step from HOST buffers: H2D of the raw arrays and D2H of every result inside ------------
     def step_host(self):
         nms, wl, h, torch = self.nms, self.wl, self.h, self.torch
-        if wl.split or len(self.rots) > 1:
+        if wl.split or len(self.rots) > 1 or self.shard is not None:
             # nms_run_host covers one rotation without object structure; here the binding-level calls are
             # used with explicit pinned copies (nms_set_sample accepts host pointers through UVA as well)
             self.d_pos.copy_(self.h_pos, non_blocking=True)
@@ -271,6 +281,50 @@ def max_over_ranks(value: float, dist=None, torch=None, dev=None) -> float:
     t = _t.tensor([float(value)], dtype=_t.float64, device=dev if dist.get_backend() == "nccl" else "cpu")
     dist.all_reduce(t, op=dist.ReduceOp.MAX)
     return float(t.item())
+
+
+def shard_lines(n0: int, world: int, rank: int):
+    """Contiguous, balanced share [i0, i1) of the n0 detector lines (rings of a polar grid, rows of a Cartesian one)
+    of rank `rank` (the detector points are independent units; the cells are replicated)."""
+    base, extra = divmod(n0, world)
+    i0 = rank * base + min(rank, extra)
+    return i0, i0 + base + (1 if rank < extra else 0)
+
+
+def shard_workload(wl, world: int, rank: int):
+    """This rank's part of a workload under line sharding: same sample, the detector lines [i0, i1)."""
+    import copy
+    g = wl.grid
+    if g.type == 2:
+        raise SystemExit("bench.py: --shard lines needs a polar or Cartesian detector")
+    if g.type == 1 and wl.n_bins:
+        raise SystemExit("bench.py: --shard lines does not cover |q| histograms on Cartesian detectors (bins straddle ranks)")
+    i0, i1 = shard_lines(g.n0, world, rank)
+    if i1 <= i0:
+        raise SystemExit("bench.py: more ranks than detector lines")
+    part = copy.copy(wl)
+    part.grid = ni.polar_grid(g.u0[i0:i1], g.n1) if g.type == 0 else ni.cartesian_grid(g.u0[i0:i1], g.u1)
+    if g.type == 0:
+        part.grid.u1 = g.u1                     # the very same float32 angles
+    part.n_bins = (i1 - i0) if wl.n_bins else 0
+    return part, i0, i1
+
+
+def gather_lines(local, n0: int, world: int, rank: int, dist):
+    """All-gather per-line results local [n_rows, n_local] (ring averages I(q_i)) into [n_rows, n0] on every rank --
+    the one exchange step of the sharded path (the Fourier-Bessel transform needs every ring).  Equal-sized padded
+    buffers, so it runs on nccl and gloo alike."""
+    import torch
+    n_max = -(-n0 // world)
+    pad = torch.zeros((local.shape[0], n_max), dtype=local.dtype, device=local.device)
+    pad[:, :local.shape[1]] = local
+    parts = [torch.empty_like(pad) for _ in range(world)]
+    dist.all_gather(parts, pad)
+    out = torch.empty((local.shape[0], n0), dtype=local.dtype, device=local.device)
+    for r in range(world):
+        i0, i1 = shard_lines(n0, world, r)
+        out[:, i0:i1] = parts[r][:, :i1 - i0]
+    return out
 
 
 def aggregate_rate(pairs_per_rank: int, world: int, ms_max: float) -> float:
@@ -393,8 +447,14 @@ def run_cuda(args, rank, local_rank, world):
     dev = torch.device("cuda", local_rank)
     torch.cuda.set_device(dev)
 
-    wl = ni.make_config(args.workload)
-    run = Runner(nms, wl, local_rank)
+    wl_full = ni.make_config(args.workload)
+    sharded = args.shard == "lines" and world > 1
+    if sharded:
+        wl, line0, line1 = shard_workload(wl_full, world, rank)
+        run = Runner(nms, wl, local_rank, shard=(wl_full, world, rank, dist))
+    else:
+        wl = wl_full
+        run = Runner(nms, wl, local_rank)
     h = run.h
     sampler = ClockSampler(local_rank)
 
@@ -413,7 +473,8 @@ def run_cuda(args, rank, local_rank, world):
            ("azimuthal", nms.NMS_T_AZIMUTHAL), ("correlation", nms.NMS_T_CORRELATION))}
     nms.nms_set_option(h, "timing", 0)
     ms_step = ms_total / args.steps
-    value = aggregate_rate(wl.pairs, world, ms_step)
+    # replicas: every rank evaluates the whole workload (weak); line sharding: the ranks share ONE workload (strong)
+    value = aggregate_rate(wl_full.pairs, 1 if sharded else world, ms_step)
 
     # ---- roofline of the dominant kernel (amplitude sums) --------------------------------------------
     peaks, peak_src = _peaks()
@@ -455,9 +516,9 @@ def run_cuda(args, rank, local_rank, world):
     e2e_steps = max(1, min(args.steps, 3))
     ms_e2e = _timed(torch, dev, run.step_host, e2e_steps, dist) / e2e_steps
     h2d, d2h = run.bytes_per_step()
-    e2e = {"value": aggregate_rate(wl.pairs, world, ms_e2e), "unit": "Gpair/s", "ms_per_step": ms_e2e,
+    e2e = {"value": aggregate_rate(wl_full.pairs, 1 if sharded else world, ms_e2e), "unit": "Gpair/s", "ms_per_step": ms_e2e,
            "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": e2e_steps}
-    next_rows = time_next_rows(nms, run, wl, torch, dev) if wl.grid.type == 0 else None
+    next_rows = time_next_rows(nms, run, wl, torch, dev) if (wl.grid.type == 0 and not sharded) else None
     run.close()
 
     cpu_baseline = None
@@ -466,9 +527,11 @@ def run_cuda(args, rank, local_rank, world):
 
     if rank == 0:
         line = {"metric": metric_name(), "value": value, "unit": "Gpair/s", "n_gpus": world, "steps": args.steps,
-                "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+                "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
+                "scaling": "strong" if sharded else "weak",
                 "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-                "config": workload_config(wl, {"parallelism": "replicas only" if world > 1 else "single GPU"}),
+                "config": workload_config(wl_full, {"parallelism": ("detector lines sharded over ranks, cells replicated, all-gather of I(q) only"
+                                                                    if sharded else "replicas only") if world > 1 else "single GPU"}),
                 "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "passes": passes,
                 "next_rows": next_rows, "cpu_baseline": cpu_baseline}
         print(json.dumps(line), flush=True)
@@ -485,6 +548,9 @@ def main():
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--oracle-seconds", type=float, default=12.0, help="CPU seconds per oracle step (bounded sample)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--shard", default="replicas", choices=["replicas", "lines"],
+                    help="N > 1: independent replicas (default, weak scaling) or the detector lines of ONE workload "
+                         "shared by the ranks (strong scaling; DESIGN.md section 9)")
     args = ap.parse_args()
     rank, local_rank, world = _env_int("RANK", 0), _env_int("LOCAL_RANK", 0), _env_int("WORLD_SIZE", 1)
     if world != args.gpus and world > 1:

@@ -18,9 +18,14 @@ dist.init_process_group(backend="gloo")
 rank, world = dist.get_rank(), dist.get_world_size()
 ms = bench.max_over_ranks(10.0 * (rank + 1), dist)          # ranks report 10 ms and 20 ms
 rate = bench.aggregate_rate(1_000_000_000, world, ms)       # 1e9 pairs per rank
+# line sharding: 7 rings over 2 ranks (4 + 3); every rank holds "I(q)" of its own rings, value = 100 * map + ring
+n0 = 7
+i0, i1 = bench.shard_lines(n0, world, rank)
+local = torch.stack([100.0 * k + torch.arange(i0, i1, dtype=torch.float32) for k in range(3)])
+full = bench.gather_lines(local, n0, world, rank, dist)
 dist.barrier()
 if rank == 0:
-    print(json.dumps({{"ms": ms, "rate": rate, "world": world}}))
+    print(json.dumps({{"ms": ms, "rate": rate, "world": world, "full": full.tolist(), "share": [i0, i1]}}))
 dist.destroy_process_group()
 """
 
@@ -38,6 +43,32 @@ def test_max_over_ranks_and_aggregate_rate_gloo(tmp_path):
     assert d["world"] == 2
     assert d["ms"] == pytest.approx(20.0)                      # the slower rank decides
     assert d["rate"] == pytest.approx(2 * 1e9 / 20e-3 / 1e9)   # both ranks' pairs over the max time
+    assert d["share"] == [0, 4]
+    assert d["full"] == [[100.0 * k + i for i in range(7)] for k in range(3)]   # rings back in detector order
+
+
+def test_line_sharding_partitions_the_detector():
+    """--shard lines: the ranks' shares are contiguous, balanced, disjoint and cover every detector line; a rank's
+    workload is the same sample on the sub-grid with the very same float32 abscissae."""
+    sys.path.insert(0, ROOT)
+    import numpy as np
+    import bench
+    import nms_inputs as ni
+    for n0 in (1, 7, 64, 512):
+        for world in (1, 2, 3, 8):
+            shares = [bench.shard_lines(n0, world, r) for r in range(world)]
+            assert shares[0][0] == 0 and shares[-1][1] == n0
+            assert all(shares[r][1] == shares[r + 1][0] for r in range(world - 1))
+            sizes = [b - a for a, b in shares]
+            assert max(sizes) - min(sizes) <= 1
+    wl = ni.make_config("C5", small=True)
+    parts = [bench.shard_workload(wl, 3, r) for r in range(3)]
+    assert np.array_equal(np.concatenate([p.grid.u0 for p, _, _ in parts]), wl.grid.u0)
+    for p, i0, i1 in parts:
+        assert p.grid.n0 == i1 - i0 and p.n_bins == i1 - i0 and np.array_equal(p.grid.u1, wl.grid.u1)
+        assert p.pos is wl.pos and p.m is wl.m                      # cells replicated, not copied
+    with pytest.raises(SystemExit):
+        bench.shard_workload(ni.make_config("C2"), 2, 0)            # |q| histogram on a Cartesian detector
 
 
 def test_single_process_helpers():

@@ -576,6 +576,48 @@ def test_cross_spectra(nms, ctx, oracle_mod, name, small):
     assert e.value.status == nms.NMS_E_ARG
 
 
+def test_bench_line_sharded_step_matches_unsharded(nms):
+    """bench.py --shard lines on one GPU: the two rank shares of the reduced C5 detector are run one after the
+    other (a stand-in process group whose all-gather returns the shares computed so far), and the assembled maps,
+    I(q) and c(r), p(r) must equal the unsharded step bit for bit (same kernels, same per-point arithmetic)."""
+    import sys, os, torch
+    sys.path.insert(0, os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
+    import bench
+    wl = ni.make_config("C5", small=True)
+    ref = bench.Runner(nms, wl, 0)
+    nms.nms_set_option(ref.h, "variant", 1)
+    ref.step_device()
+    nms.nms_synchronize(ref.h)
+    world = 2
+
+    class StandIn:                      # all_gather over shares that were computed sequentially on this one GPU
+        def __init__(self):
+            self.store = {}
+            self.rank = 0
+        def all_gather(self, parts, pad):
+            self.store[self.rank] = pad.clone()
+            for r in range(world):
+                parts[r].copy_(self.store.get(r, torch.zeros_like(pad)))
+
+    dist = StandIn()
+    maps = torch.empty_like(ref.maps)
+    c_last = p_last = None
+    for rank in (0, 1):
+        dist.rank = rank
+        part, i0, i1 = bench.shard_workload(wl, world, rank)
+        run = bench.Runner(nms, part, 0, shard=(wl, world, rank, dist))
+        nms.nms_set_option(run.h, "variant", 1)
+        run.step_device()
+        nms.nms_synchronize(run.h)
+        maps[:, i0 * wl.grid.n1:i1 * wl.grid.n1] = run.maps
+        assert torch.equal(run.I, ref.I[:, i0:i1])
+        c_last, p_last = run.c.clone(), run.p.clone()
+        run.close()
+    assert torch.equal(maps, ref.maps)
+    assert torch.equal(c_last, ref.c) and torch.equal(p_last, ref.p)     # the last rank saw every ring
+    ref.close()
+
+
 def test_histogram_on_polar_grid_and_empty_bins(nms, ctx, oracle_mod):
     import torch
     wl = ni.make_config("C1")
