@@ -365,8 +365,35 @@ def oracle_sample(wl, n_sample):
     return ni.q_subset(wl.grid.n_q, n, 9000 + (int(wl.name[1]) if wl.name[1].isdigit() else 0))
 
 
-def time_oracle(wl, target_s=12.0, steps=1, warmup=0):
-    """Gpair/s of the oracle on a sample sized for about target_s seconds per step (probe first, then scale)."""
+def parity_report(wl, maps_gpu, idx, M_ref):
+    """Worst relative deviation of the step's GPU maps from the oracle maps on the timed sample of detector points,
+    wherever |oracle| > 1e-6 of the GPU map's maximum (north_star criterion); the signed kinds NM and CHI are
+    reported separately above 1e-5 of their parents' maxima (reading 16)."""
+    names = [ni.KINDS[k] for k in wl.kinds]
+    fmax = np.abs(maps_gpu).max(axis=1)
+    def mx(name):
+        return fmax[names.index(name)] if name in names else 0.0
+    parent = {"NM": mx("NUC") + mx("PROJ"), "CHI": mx("SF")}
+    worst_pos, worst_signed = 0.0, 0.0
+    for i, name in enumerate(names):
+        floor = 1e-6 * fmax[i]
+        if name in parent:
+            floor = max(floor, 1e-5 * parent[name])
+        sel = np.abs(M_ref[i]) > floor
+        if not sel.any():
+            continue
+        rel = float((np.abs(maps_gpu[i][idx][sel] - M_ref[i][sel]) / np.abs(M_ref[i][sel])).max())
+        if name in parent:
+            worst_signed = max(worst_signed, rel)
+        else:
+            worst_pos = max(worst_pos, rel)
+    return {"points": int(len(idx)), "max_rel_err_positive_kinds": worst_pos, "max_rel_err_signed_kinds": worst_signed,
+            "tolerance": 1e-3}
+
+
+def time_oracle(wl, target_s=12.0, steps=1, warmup=0, keep=None):
+    """Gpair/s of the oracle on a sample sized for about target_s seconds per step (probe first, then scale).
+    keep: dict that receives the sample indices and the oracle maps of the last step (for the parity report)."""
     import oracle
     oracle.build()
     qy, qz, th = oracle.grid_points(wl.grid)
@@ -386,8 +413,10 @@ def time_oracle(wl, target_s=12.0, steps=1, warmup=0):
         oracle_step(oracle, wl, qy, qz, th, idx)
     t0 = time.perf_counter()
     for _ in range(steps):
-        oracle_step(oracle, wl, qy, qz, th, idx)
+        M = oracle_step(oracle, wl, qy, qz, th, idx)
     dt = (time.perf_counter() - t0) / steps
+    if keep is not None:
+        keep["idx"], keep["M"] = idx, M
     pairs = wl.W * len(idx)
     return {"value": pairs / dt / 1e9, "unit": "Gpair/s", "cores": oracle.num_threads(), "kind": "oracle",
             "sample": f"all {wl.W} cells x {len(idx)} of {wl.grid.n_q} detector points (seeded subset, first rotation), "
@@ -519,11 +548,15 @@ def run_cuda(args, rank, local_rank, world):
     e2e = {"value": aggregate_rate(wl_full.pairs, 1 if sharded else world, ms_e2e), "unit": "Gpair/s", "ms_per_step": ms_e2e,
            "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": e2e_steps}
     next_rows = time_next_rows(nms, run, wl, torch, dev) if (wl.grid.type == 0 and not sharded) else None
+    maps_host = run.maps.cpu().numpy().astype(np.float64) if wl.n_rot == 1 else None   # the last step's maps
     run.close()
 
-    cpu_baseline = None
+    cpu_baseline, parity = None, None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        cpu_baseline, _ = time_oracle(wl, target_s=args.oracle_seconds)
+        keep = {}
+        cpu_baseline, _ = time_oracle(wl, target_s=args.oracle_seconds, keep=keep)
+        if maps_host is not None:                       # the oracle sample doubles as a parity check of this very run
+            parity = parity_report(wl, maps_host, keep["idx"], keep["M"])
 
     if rank == 0:
         line = {"metric": metric_name(), "value": value, "unit": "Gpair/s", "n_gpus": world, "steps": args.steps,
@@ -533,7 +566,7 @@ def run_cuda(args, rank, local_rank, world):
                 "config": workload_config(wl_full, {"parallelism": ("detector lines sharded over ranks, cells replicated, all-gather of I(q) only"
                                                                     if sharded else "replicas only") if world > 1 else "single GPU"}),
                 "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "passes": passes,
-                "next_rows": next_rows, "cpu_baseline": cpu_baseline}
+                "next_rows": next_rows, "cpu_baseline": cpu_baseline, "parity": parity}
         print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()
