@@ -3,8 +3,8 @@
 //  prep kernel   (Eq. 37-41):  r' = R (x + r^k), m' = R m in fp64; only Y, Z (rows 2, 3 of R)
 //                are kept because q_x = 0 on the detector (Eq. 41).  One block per tile, TILE/256 cells per
 //                thread: it writes the Cell records (fp64 Y, Z; weights rounded once to fp32), finds
-//                the tile's bounding-box midpoint (Y0, Z0) and extent, and accumulates sum_j |w_cj| for
-//                the tolerance denominators.
+//                the tile's bounding-box midpoint (Y0, Z0) and extent, and writes the tile's sum_j |w_cj|;
+//                k_wsum_reduce adds the tiles in a fixed order (the tolerance denominators, deterministic).
 //  qsetup kernel (Eq. 6): per detector point (q_y, q_z) in fp64 [rad/nm] and
 //                (sin th, cos th) for the response epilogue.
 #include "nms_internal.h"
@@ -24,7 +24,7 @@ struct PrepArgs {
     const int32_t* flags;
     TileMeta* meta;
     Cell* cells;
-    double* wsum;
+    double* tile_wsum;   // [n_tiles][4]: per-tile sum_j |w_cj| (reduced by k_wsum_reduce)
     double R[9];
 };
 
@@ -110,8 +110,7 @@ __global__ void __launch_bounds__(PREP_THREADS) k_prep(const PrepArgs a)
         tm.ext = ts.n_src > 0 ? (float)fmax(0.5 * (v[1] - v[0]), 0.5 * (v[3] - v[2])) : 0.f;
         tm.pad_ = 0;
         a.meta[tile] = tm;
-        for (int r = 0; r < 4; ++r)
-            if (v[4 + r] != 0.0) atomicAdd(a.wsum + r, v[4 + r]);
+        for (int r = 0; r < 4; ++r) a.tile_wsum[4 * (int64_t)tile + r] = v[4 + r];
     }
 #pragma unroll
     for (int u = 0; u < PREP_PER_THREAD; ++u) {
@@ -122,6 +121,29 @@ __global__ void __launch_bounds__(PREP_THREADS) k_prep(const PrepArgs a)
             ce.wN = wN[u]; ce.wx = wx[u]; ce.wy = wy[u]; ce.wz = wz[u];
             a.cells[first_slot + i] = ce;
         }
+    }
+}
+
+// sum_j |w_cj| over all tiles: one block, fixed order (deterministic, unlike atomics on four addresses)
+__global__ void __launch_bounds__(1024) k_wsum_reduce(const double* __restrict__ tile_wsum, int64_t n_tiles,
+                                                      double* __restrict__ wsum)
+{
+    __shared__ double red[4][32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    double s[4] = {0.0, 0.0, 0.0, 0.0};
+    for (int64_t t = threadIdx.x; t < n_tiles; t += blockDim.x)
+#pragma unroll
+        for (int r = 0; r < 4; ++r) s[r] += tile_wsum[4 * t + r];
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+        s[r] = warp_sum(s[r]);
+        if (lane == 0) red[r][warp] = s[r];
+    }
+    __syncthreads();
+    if (threadIdx.x < 4) {
+        double v = 0.0;
+        for (int w = 0; w < 32; ++w) v += red[threadIdx.x][w];
+        wsum[threadIdx.x] = v;
     }
 }
 
@@ -139,13 +161,14 @@ nms_status launch_prep(nms_ctx* c)
     a.flags = (const int32_t*)(base + sizeof(int64_t) * (size_t)c->n_tiles);
     a.meta = (TileMeta*)c->tile_meta.p;
     a.cells = (Cell*)c->cells.p;
-    a.wsum = (double*)c->wsum.p;
+    if (nms_status st = ensure(c, c->tile_wsum, sizeof(double) * 4 * (size_t)c->n_tiles)) return st;
+    a.tile_wsum = (double*)c->tile_wsum.p;
     for (int i = 0; i < 9; ++i) a.R[i] = c->R[i];
-    NMS_CUDA(c, cudaMemsetAsync(c->wsum.p, 0, 4 * sizeof(double), c->stream));
     timer_begin(c, NMS_T_PREP);
     k_prep<<<(unsigned)c->n_tiles, PREP_THREADS, 0, c->stream>>>(a);
+    k_wsum_reduce<<<1, 1024, 0, c->stream>>>((const double*)c->tile_wsum.p, c->n_tiles, (double*)c->wsum.p);
     timer_end(c, NMS_T_PREP);
-    c->launches += 1;
+    c->launches += 2;
     NMS_CUDA(c, cudaGetLastError());
     return NMS_OK;
 }

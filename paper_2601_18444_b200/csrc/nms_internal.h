@@ -83,6 +83,7 @@ struct nms_ctx {
     std::vector<nms::TileSrc> h_tile_src;
     std::vector<int32_t> h_tile_flags;
     std::vector<int64_t> h_tile_first_slot;
+    nms::DevBuf tile_wsum;             // double [n_tiles][4]: per-tile sum |w|
     nms::DevBuf tile_src, tile_meta, cells, wsum;   // cells: Cell[n_slots]; wsum: double[4]
 
     // current detector grid
