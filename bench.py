@@ -463,6 +463,32 @@ def run_reference(args, rank):
     print(json.dumps(line), flush=True)
 
 
+def run_sweep(args):
+    """Context measurement, not the contract line: the paper's runtime experiment (Fig. 10) re-created
+    synthetically -- step time against the number of cells for K = 10 ... 25 600 identical vortex spheres of 4169
+    cells (ni.config_fig10), all 13 responses + ring average + c(r), p(r) on a 256 x 256 polar detector."""
+    import torch
+    import paper_2601_18444_b200 as nms
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    points = []
+    for K in (10, 40, 160, 640, 2560, 10240, 25600):
+        wl = ni.config_fig10(K)
+        run = Runner(nms, wl, 0)
+        for _ in range(2):
+            run.step_device()
+        steps = 3 if K <= 2560 else 2
+        ms = _timed(torch, dev, run.step_device, steps) / steps
+        points.append({"particles": K, "cells": wl.W, "ms_per_step": ms, "gpair_s": wl.pairs / (ms * 1e-3) / 1e9,
+                       "variant": nms.nms_get_info(run.h, "variant_used")})
+        run.close()
+        del run, wl
+        torch.cuda.empty_cache()
+    print(json.dumps({"sweep": "fig10", "detector": "polar 256x256, |q| 0.01-1.5 linear", "kinds": 13,
+                      "note": "whole step per point: prep + amplitudes + responses + I(q) + c(r), p(r); inputs resident",
+                      "points": points}), flush=True)
+
+
 def run_cuda(args, rank, local_rank, world):
     import torch
     if not torch.cuda.is_available():
@@ -581,6 +607,8 @@ def main():
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--oracle-seconds", type=float, default=12.0, help="CPU seconds per oracle step (bounded sample)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep", action="store_true",
+                    help="context only: step time against cell count for the paper's Fig. 10 workload (one JSON line)")
     ap.add_argument("--shard", default="replicas", choices=["replicas", "lines"],
                     help="N > 1: independent replicas (default, weak scaling) or the detector lines of ONE workload "
                          "shared by the ranks (strong scaling; DESIGN.md section 9)")
@@ -590,7 +618,10 @@ def main():
         raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}")
     if args.gpus > 1 and world == 1:
         raise SystemExit("bench.py: for --gpus N > 1 launch with python -m torch.distributed.run --nproc-per-node N")
-    if args.impl == "reference":
+    if args.sweep:
+        if rank == 0:
+            run_sweep(args)
+    elif args.impl == "reference":
         run_reference(args, rank)
     else:
         run_cuda(args, rank, local_rank, world)

@@ -269,6 +269,27 @@ def config_sec4c(K: int = 800, n_q: int = 1000, n_theta: int = 1000) -> Workload
                     n_bins=n_q, r=np.linspace(0.0, 30.0, 512).astype(np.float32))
 
 
+def config_fig10(K: int, n_q: int = 256, n_theta: int = 256) -> Workload:
+    """Context workload, not a BASELINE.json config: synthetic re-creation of the paper's runtime experiment
+    (Sec. IV D, Eq. 109): K identical spheres D = 40 nm on a node-centred a = 2 nm lattice (4169 cells
+    each), linear vortex m = (-5y/R, 5x/R, 1)/|.| in the particle's own frame, uniform N = 1; centres on a simple
+    cubic lattice of 60 nm (the paper does not say where its copies sit); polar detector, |q| linear in 0.01-1.5."""
+    local = sphere_node_centred(20.0, 2.0)
+    x, y = local[:, 0] / 20.0, local[:, 1] / 20.0
+    mv = np.stack([-5.0 * y, 5.0 * x, np.ones_like(x)], axis=1)
+    mv /= np.linalg.norm(mv, axis=1, keepdims=True)
+    n_side = int(np.ceil(K ** (1.0 / 3.0)))
+    idx = np.arange(K)
+    cen = np.stack([idx % n_side, (idx // n_side) % n_side, idx // (n_side * n_side)], axis=1).astype(np.float64)
+    cen = (cen - 0.5 * (n_side - 1)) * 60.0
+    pos = (cen[:, None, :] + local[None, :, :]).reshape(-1, 3).astype(np.float32)
+    W = pos.shape[0]
+    q = 0.01 + 1.49 * np.arange(n_q, dtype=np.float64) / max(n_q - 1, 1)
+    return Workload(name="F10", pos=pos, N=np.ones(W, dtype=np.float32), m=np.tile(mv.astype(np.float32), (K, 1)),
+                    grid=polar_grid(q, n_theta), kinds=list(ALL_KINDS), n_bins=n_q,
+                    r=np.linspace(0.0, 60.0, 256).astype(np.float32))
+
+
 def config_c4(nx: int = 512, ny: int = 512, nz: int = 8, n_rot: int = 36, n_grid: int = 256) -> Workload:
     """Neel-skyrmion-lattice film, hexagonal lattice period 50 nm; rocking scan about z in 10 degree steps."""
     x = np.arange(nx, dtype=np.float64) + 0.5 - nx / 2.0
