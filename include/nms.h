@@ -232,7 +232,8 @@ NMS_API nms_status nms_get_weight_sums(nms_ctx* ctx, double* out);
  * u0 is not an arithmetic progression within one fp32 ulp), 3 force the exact fp64 kernel.  "bases": exactly
  * evaluated points per 8 in the recurrence kernel (0 auto = 2, else 1..4).  "timing": 1 records a CUDA
  * event pair around every kernel launch (and resets the record).  "chunks": 0 auto, else the number of cell
- * chunks.  "qt": 0 auto, else detector points per thread (4 or 8).  Unknown keys: NMS_E_ARG.            */
+ * chunks.  "qt": 0 auto, else detector points per thread (4 or 8; 16 for the recurrence kernel on a sample
+ * without moments).  Unknown keys: NMS_E_ARG.                                                            */
 NMS_API nms_status nms_set_option(nms_ctx* ctx, const char* key, int64_t value);
 /* Read back integers: "launches" (kernels launched by this context so far), "variant_used" (1 list direct,
  * 2 polar direct, 4 cartesian direct, 3 polar recurrence, 5 cartesian recurrence, 8 exact fp64),

@@ -442,8 +442,10 @@ static amp_kernel_t pick_split(bool split, bool nuclear_only)
 }
 
 template <int MODE>
-static amp_kernel_t pick_rec(int nb, bool split, bool nuc)
+static amp_kernel_t pick_rec(int qt, int nb, bool split, bool nuc)
 {
+    // one channel leaves room for 16 points per thread: the phasor set-up per pair halves (bases stay <= 2 steps away)
+    if (qt == 16) return split ? (amp_kernel_t)k_amp<MODE, 16, true, 4, 4, 1> : (amp_kernel_t)k_amp<MODE, 16, false, 4, 4, 1>;
     switch (nb) {
     case 1: return pick_split<MODE, 8, 4, 1>(split, nuc);
     case 3: return pick_split<MODE, 8, 4, 3>(split, nuc);
@@ -464,8 +466,8 @@ static amp_kernel_t pick_kernel(int variant, int qt, int nb, bool split, bool nu
     case 4:
         if (qt == 4) return pick_split<1, 4, 4, 0>(split, nuc);
         return pick_split<1, 8, 4, 0>(split, nuc);
-    case 3: return pick_rec<0>(nb, split, nuc);
-    case 5: return pick_rec<1>(nb, split, nuc);
+    case 3: return pick_rec<0>(qt, nb, split, nuc);
+    case 5: return pick_rec<1>(qt, nb, split, nuc);
     default: return split ? (amp_kernel_t)k_amp_f64<true> : (amp_kernel_t)k_amp_f64<false>;
     }
 }
@@ -493,7 +495,7 @@ nms_status plan_amplitude(nms_ctx* c, bool split, AmpPlan* plan)
     int qt_opts[3]; int n_opts = 0;
     if (variant == 8) { qt_opts[n_opts++] = 1; }
     else if (variant == 1) { qt_opts[n_opts++] = 4; }
-    else if (variant == 3 || variant == 5) { qt_opts[n_opts++] = 8; }
+    else if (variant == 3 || variant == 5) { if (!c->has_M && c->opt_bases == 0) qt_opts[n_opts++] = 16; qt_opts[n_opts++] = 8; }
     else { qt_opts[n_opts++] = 8; qt_opts[n_opts++] = 4; }
     int qt = qt_opts[n_opts - 1];
     if (c->opt_qt && variant != 8) {

@@ -489,7 +489,7 @@ nms_status nms_set_option(nms_ctx* c, const char* key, int64_t value)
     else if (!strcmp(key, "timing")) { c->opt_timing = value != 0; for (Timer& t : c->timers) t.used = 0; }
     else if (!strcmp(key, "chunks")) { if (value < 0) return fail(c, NMS_E_ARG, "chunks must be >= 0"); c->opt_chunks = (int)value; }
     else if (!strcmp(key, "bases")) { if (value < 0 || value > 4) return fail(c, NMS_E_ARG, "bases must be 0..4"); c->opt_bases = (int)value; }
-    else if (!strcmp(key, "qt")) { if (value != 0 && value != 4 && value != 8) return fail(c, NMS_E_ARG, "qt must be 0, 4 or 8"); c->opt_qt = (int)value; }
+    else if (!strcmp(key, "qt")) { if (value != 0 && value != 4 && value != 8 && value != 16) return fail(c, NMS_E_ARG, "qt must be 0, 4, 8 or 16"); c->opt_qt = (int)value; }
     else return fail(c, NMS_E_ARG, "unknown option '%s'", key);
     return NMS_OK;
 }

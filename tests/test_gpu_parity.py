@@ -527,6 +527,8 @@ def test_activation_switches(nms, ctx, oracle_mod, which, variant):
     kinds = [KI["NUC"], KI["MAG"], KI["UNPOL"], KI["SF"]]
     nms.nms_set_sample(ctx, _t(wl.pos), _t(N), _t(m), wl.R)
     nms.nms_set_option(ctx, "variant", variant)
+    if which == "nuclear_only" and variant == 2:
+        nms.nms_set_option(ctx, "qt", 16)                          # the 16-points-per-thread one-channel recurrence
     amp = torch.empty((8, wl.grid.n_q), dtype=torch.float32, device="cuda")
     maps = torch.empty((len(kinds), wl.grid.n_q), dtype=torch.float32, device="cuda")
     nms.nms_amplitudes(ctx, wl.grid, amp)
@@ -536,6 +538,8 @@ def test_activation_switches(nms, ctx, oracle_mod, which, variant):
     A, wsum = oracle_mod.amplitudes(wl.pos, N, m, wl.R, qy, qz, return_wsum=True)
     M = oracle_mod.response(A, th, kinds, P=wl.P)
     assert_amplitudes(amp.cpu().numpy(), A, wsum, which)
+    if which == "nuclear_only" and variant == 2:
+        assert nms.nms_get_info(ctx, "qt") == 16
     got = maps.cpu().numpy()
     live = [0, 2] if which == "nuclear_only" else [1, 2, 3]
     assert_cross_sections(got[live], M[live], [kinds[i] for i in live], which)
