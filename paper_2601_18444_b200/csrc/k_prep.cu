@@ -2,8 +2,7 @@
 //
 //  prep kernel   (Eq. 37-41):  r' = R (x + r^k), m' = R m in fp64; only Y, Z (rows 2, 3 of R)
 //                are kept because q_x = 0 on the detector (Eq. 41).  One block per tile, TILE/256 cells per
-//                thread: it writes the Cell records (fp64 Y, Z; weights rounded once to fp32), finds
-//                the tile's bounding-box midpoint (Y0, Z0) and extent, and writes the tile's sum_j |w_cj|;
+//                thread: it writes the Cell records (fp64 Y, Z; weights rounded once to fp32) and the tile's sum_j |w_cj|;
 //                k_wsum_reduce adds the tiles in a fixed order (the tolerance denominators, deterministic).
 //  qsetup kernel (Eq. 6): per detector point (q_y, q_z) in fp64 [rad/nm] and
 //                (sin th, cos th) for the response epilogue.
@@ -28,16 +27,6 @@ struct PrepArgs {
     double R[9];
 };
 
-__device__ __forceinline__ double warp_min(double v)
-{
-    for (int o = 16; o > 0; o >>= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, o));
-    return v;
-}
-__device__ __forceinline__ double warp_max(double v)
-{
-    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
-    return v;
-}
 __device__ __forceinline__ double warp_sum(double v)
 {
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
@@ -46,7 +35,7 @@ __device__ __forceinline__ double warp_sum(double v)
 
 __global__ void __launch_bounds__(PREP_THREADS) k_prep(const PrepArgs a)
 {
-    __shared__ double red[8][PREP_THREADS / 32];
+    __shared__ double red[4][PREP_THREADS / 32];
     const int tile = blockIdx.x;
     const TileSrc ts = a.src[tile];
     const int64_t first_slot = a.first_slot[tile];
@@ -61,7 +50,6 @@ __global__ void __launch_bounds__(PREP_THREADS) k_prep(const PrepArgs a)
     }
     double Y[PREP_PER_THREAD], Z[PREP_PER_THREAD];
     float wN[PREP_PER_THREAD], wx[PREP_PER_THREAD], wy[PREP_PER_THREAD], wz[PREP_PER_THREAD];
-    double ymin = INFINITY, ymax = -INFINITY, zmin = INFINITY, zmax = -INFINITY;
     double sN = 0.0, sx = 0.0, sy = 0.0, sz = 0.0;
 #pragma unroll
     for (int u = 0; u < PREP_PER_THREAD; ++u) {
@@ -75,8 +63,6 @@ __global__ void __launch_bounds__(PREP_THREADS) k_prep(const PrepArgs a)
             const double z = (double)a.pos[3 * j + 2] + cz;
             Y[u] = a.R[3] * x + a.R[4] * y + a.R[5] * z;   // Eq. 39
             Z[u] = a.R[6] * x + a.R[7] * y + a.R[8] * z;   // Eq. 40
-            ymin = fmin(ymin, Y[u]); ymax = fmax(ymax, Y[u]);
-            zmin = fmin(zmin, Z[u]); zmax = fmax(zmax, Z[u]);
             if (a.N) { wN[u] = a.N[j]; sN += fabs((double)wN[u]); }
             if (a.m) {
                 const double mx = (double)a.m[3 * j + 0], my = (double)a.m[3 * j + 1], mz = (double)a.m[3 * j + 2];
@@ -88,29 +74,21 @@ __global__ void __launch_bounds__(PREP_THREADS) k_prep(const PrepArgs a)
             }
         }
     }
-    ymin = warp_min(ymin); ymax = warp_max(ymax); zmin = warp_min(zmin); zmax = warp_max(zmax);
     sN = warp_sum(sN); sx = warp_sum(sx); sy = warp_sum(sy); sz = warp_sum(sz);
     if (lane == 0) {
-        red[0][warp] = ymin; red[1][warp] = ymax; red[2][warp] = zmin; red[3][warp] = zmax;
-        red[4][warp] = sN; red[5][warp] = sx; red[6][warp] = sy; red[7][warp] = sz;
+        red[0][warp] = sN; red[1][warp] = sx; red[2][warp] = sy; red[3][warp] = sz;
     }
     __syncthreads();
     if (tid == 0) {
-        double v[8];
-        for (int r = 0; r < 8; ++r) v[r] = red[r][0];
-        for (int w = 1; w < PREP_THREADS / 32; ++w) {
-            v[0] = fmin(v[0], red[0][w]); v[1] = fmax(v[1], red[1][w]);
-            v[2] = fmin(v[2], red[2][w]); v[3] = fmax(v[3], red[3][w]);
-            for (int r = 4; r < 8; ++r) v[r] += red[r][w];
-        }
-        const double Y0 = ts.n_src > 0 ? 0.5 * (v[0] + v[1]) : 0.0;
-        const double Z0 = ts.n_src > 0 ? 0.5 * (v[2] + v[3]) : 0.0;
+        double v[4];
+        for (int r = 0; r < 4; ++r) v[r] = red[r][0];
+        for (int w = 1; w < PREP_THREADS / 32; ++w)
+            for (int r = 0; r < 4; ++r) v[r] += red[r][w];
         TileMeta tm;
-        tm.Y0 = Y0; tm.Z0 = Z0; tm.first_slot = first_slot; tm.n_slots = n_slots; tm.flags = a.flags[tile];
-        tm.ext = ts.n_src > 0 ? (float)fmax(0.5 * (v[1] - v[0]), 0.5 * (v[3] - v[2])) : 0.f;
-        tm.pad_ = 0;
+        tm.Y0 = 0.0; tm.Z0 = 0.0; tm.first_slot = first_slot; tm.n_slots = n_slots; tm.flags = a.flags[tile];
+        tm.ext = 0.f; tm.pad_ = 0;
         a.meta[tile] = tm;
-        for (int r = 0; r < 4; ++r) a.tile_wsum[4 * (int64_t)tile + r] = v[4 + r];
+        for (int r = 0; r < 4; ++r) a.tile_wsum[4 * (int64_t)tile + r] = v[r];
     }
 #pragma unroll
     for (int u = 0; u < PREP_PER_THREAD; ++u) {

@@ -26,11 +26,11 @@ struct Cell {              // 32 B, the unit of the bulk copies (16-byte aligned
 };
 
 struct TileMeta {          // consumed by the amplitude kernel
-    double Y0, Z0;         // bounding-box midpoint [nm] (origin of the line-recurrence kernel)
+    double Y0, Z0;         // reserved (tile origin; unused: phases are reduced exactly in fp64)
     int64_t first_slot;    // index into the cell array
     int32_t n_slots;       // cell count of the tile
     int32_t flags;         // bit 0: last tile of its object, bit 1: first tile (form-factor split)
-    float ext;             // max over the tile's cells of |Y - Y0|, |Z - Z0| [nm]
+    float ext;             // reserved
     int32_t pad_;
 };
 struct TileSrc {           // consumed by the prep kernel
