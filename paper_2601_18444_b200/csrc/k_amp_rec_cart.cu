@@ -1,0 +1,34 @@
+// k_amp_rec_cart.cu -- instantiations of the line-recurrence amplitude kernels (k_amplitude.cuh, NB > 0) for
+// MODE = 1 (cart detector): NB exactly evaluated points per QT, rotations or the three-term recurrence, phasors of
+// the bases and of the step by MUFU or by polynomial.
+#include "k_amplitude.cuh"
+
+namespace nms {
+
+template <int QT, int NB, int NCH, int REC3>
+static amp_kernel_t pick(bool split, bool poly)
+{
+    if constexpr (NCH == 4) if (split)
+        return poly ? (amp_kernel_t)k_amp<1, QT, true, 4, NB, 4, 1, REC3> : (amp_kernel_t)k_amp<1, QT, true, 4, NB, 4, 0, REC3>;
+    return poly ? (amp_kernel_t)k_amp<1, QT, false, 4, NB, NCH, 1, REC3> : (amp_kernel_t)k_amp<1, QT, false, 4, NB, NCH, 0, REC3>;
+}
+
+amp_kernel_t amp_kernel_rec_cart(int qt, int nb, bool split, int nch, bool poly, bool rec3)
+{
+    if (nch == 1) {
+        if (split) return nullptr;
+        if (qt == 16 && nb == 4) return rec3 ? pick<16, 4, 1, 1>(false, poly) : pick<16, 4, 1, 0>(false, poly);
+        if (qt == 8 && nb == 2) return rec3 ? pick<8, 2, 1, 1>(false, poly) : pick<8, 2, 1, 0>(false, poly);
+        return nullptr;
+    }
+    if (qt != 8) return nullptr;
+    switch (nb) {
+    case 1: return rec3 ? pick<8, 1, 4, 1>(split, poly) : pick<8, 1, 4, 0>(split, poly);
+    case 2: return rec3 ? pick<8, 2, 4, 1>(split, poly) : pick<8, 2, 4, 0>(split, poly);
+    case 3: return rec3 ? nullptr : pick<8, 3, 4, 0>(split, poly);
+    case 4: return rec3 ? nullptr : pick<8, 4, 4, 0>(split, poly);
+    default: return nullptr;
+    }
+}
+
+}  // namespace nms

@@ -84,9 +84,9 @@ __global__ void __launch_bounds__(256) k_cross_spectra(const double* __restrict_
 nms_status launch_cross_spectra(nms_ctx* c, float* out_GR, float* out_GI)
 {
     const unsigned blocks = (unsigned)((c->n_q + 255) / 256);
-    timer_begin(c, NMS_T_EPILOGUE);
+    if (nms_status ts_ = timer_begin(c, NMS_T_EPILOGUE)) return ts_;
     k_cross_spectra<<<blocks, 256, 0, c->stream>>>((const double*)c->amp64.p, c->n_q, c->invV * c->sM * c->sM, out_GR, out_GI);
-    timer_end(c, NMS_T_EPILOGUE);
+    if (nms_status ts_ = timer_end(c, NMS_T_EPILOGUE)) return ts_;
     c->launches += 1;
     NMS_CUDA(c, cudaGetLastError());
     return NMS_OK;
@@ -102,9 +102,9 @@ static nms_status run(nms_ctx* c, const EpiArgs& a)
 {
     const int threads = 256;
     const unsigned blocks = (unsigned)((c->n_q + threads - 1) / threads);
-    timer_begin(c, NMS_T_EPILOGUE);
+    if (nms_status ts_ = timer_begin(c, NMS_T_EPILOGUE)) return ts_;
     k_epilogue<<<blocks, threads, 0, c->stream>>>(a);
-    timer_end(c, NMS_T_EPILOGUE);
+    if (nms_status ts_ = timer_end(c, NMS_T_EPILOGUE)) return ts_;
     c->launches += 1;
     NMS_CUDA(c, cudaGetLastError());
     return NMS_OK;

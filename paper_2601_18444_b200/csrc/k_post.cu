@@ -115,7 +115,7 @@ nms_status launch_modal(nms_ctx* c, const float* maps, int n_maps, int k_max, fl
     const int nk = k_max + 1, n0 = c->g_n0, n1 = c->g_n1;
     if (nms_status st = ensure(c, c->modal_tab, sizeof(double2) * (size_t)nk * n1)) return st;
     if (nms_status st = ensure(c, c->modal_ring, sizeof(double2) * (size_t)n_maps * nk * n0)) return st;
-    timer_begin(c, NMS_T_MODAL);
+    if (nms_status ts_ = timer_begin(c, NMS_T_MODAL)) return ts_;
     k_modal_table<<<(unsigned)((nk * n1 + 255) / 256), 256, 0, c->stream>>>((const float*)c->u1.p, n1, nk,
                                                                            (double2*)c->modal_tab.p);
     const int64_t warps = (int64_t)n_maps * nk * n0;
@@ -127,7 +127,7 @@ nms_status launch_modal(nms_ctx* c, const float* maps, int n_maps, int k_max, fl
         k_modal_amplitudes<<<(unsigned)n_maps, 1024, 0, c->stream>>>((const double2*)c->modal_ring.p, n0, nk, out_a, out_A);
         c->launches += 1;
     }
-    timer_end(c, NMS_T_MODAL);
+    if (nms_status ts_ = timer_end(c, NMS_T_MODAL)) return ts_;
     NMS_CUDA(c, cudaGetLastError());
     return NMS_OK;
 }
@@ -192,7 +192,7 @@ __global__ void __launch_bounds__(256) k_bin_finish(const double* __restrict__ b
 nms_status launch_azimuthal(nms_ctx* c, const float* maps, int n_maps, int n_bins, double q_lo, double q_hi,
                             float* out_I, float* out_q, int32_t* out_count)
 {
-    timer_begin(c, NMS_T_AZIMUTHAL);
+    if (nms_status ts_ = timer_begin(c, NMS_T_AZIMUTHAL)) return ts_;
     if (c->g_type == 0 && !(q_hi > q_lo)) {
         const int64_t warps = (int64_t)n_maps * c->g_n0;
         const unsigned blocks = (unsigned)((warps * 32 + 255) / 256);
@@ -216,7 +216,7 @@ nms_status launch_azimuthal(nms_ctx* c, const float* maps, int n_maps, int n_bin
                                                 n_bins, q_lo, q_hi, out_I, out_q, out_count);
         c->launches += 3;
     }
-    timer_end(c, NMS_T_AZIMUTHAL);
+    if (nms_status ts_ = timer_end(c, NMS_T_AZIMUTHAL)) return ts_;
     NMS_CUDA(c, cudaGetLastError());
     return NMS_OK;
 }
@@ -249,7 +249,7 @@ __global__ void __launch_bounds__(256) k_pixel_cells(const float* __restrict__ m
     if (p % TILE == 0 && p < n) {
         TileMeta tm;
         tm.Y0 = 0.0; tm.Z0 = 0.0; tm.first_slot = p; tm.n_slots = (int32_t)((n - p) < TILE ? (n - p) : TILE);
-        tm.flags = 3; tm.ext = 0.f; tm.pad_ = 0;
+        tm.flags = 3;
         meta[p / TILE] = tm;
     }
 }
@@ -284,9 +284,11 @@ nms_status launch_correlation_2d(nms_ctx* c, const float* map, const nms_qgrid* 
     struct Saved {
         DevBuf cells, tile_meta, u0, u1, qc, sc;
         int64_t n_tiles, n_slots, W, K, n_q;
-        bool grid_valid, g_uniform, has_N, has_M;
-        int g_type, g_n0, g_n1;
-        double g_dq;
+        bool grid_valid, g_uniform, has_N, has_M, amp_valid;
+        int g_type, g_n0, g_n1, opt_qt, opt_bases, amp_timer;
+        int variant_used, n_chunks_used, blocks_per_sm_used, qt_used, npoly_used, nb_used, rec3_used;
+        double g_dq, g_dev, g_qmax, geo_rmax, geo_ext, geo_extz;
+        bool geo_pending;
         std::vector<float> h_u0, h_u1;
     } sv;
     auto exchange = [&]() {
@@ -297,27 +299,44 @@ nms_status launch_correlation_2d(nms_ctx* c, const float* map, const nms_qgrid* 
         std::swap(sv.has_N, c->has_N); std::swap(sv.has_M, c->has_M);
         std::swap(sv.g_type, c->g_type); std::swap(sv.g_n0, c->g_n0); std::swap(sv.g_n1, c->g_n1); std::swap(sv.g_dq, c->g_dq);
         std::swap(sv.h_u0, c->h_u0); std::swap(sv.h_u1, c->h_u1);
+        // the caller's stored amplitudes, tuning options and "used" records survive the exchanged run; the inner
+        // amplitude launch is timed under NMS_T_CORR2D only
+        std::swap(sv.amp_valid, c->amp_valid); std::swap(sv.opt_qt, c->opt_qt); std::swap(sv.opt_bases, c->opt_bases);
+        std::swap(sv.amp_timer, c->amp_timer);
+        std::swap(sv.g_dev, c->g_dev); std::swap(sv.g_qmax, c->g_qmax); std::swap(sv.geo_rmax, c->geo_rmax);
+        std::swap(sv.geo_ext, c->geo_ext); std::swap(sv.geo_extz, c->geo_extz); std::swap(sv.geo_pending, c->geo_pending);
+    };
+    auto keep_used = [&](bool save) {
+        int* u[] = {&c->variant_used, &c->n_chunks_used, &c->blocks_per_sm_used, &c->qt_used, &c->npoly_used, &c->nb_used, &c->rec3_used};
+        int* s[] = {&sv.variant_used, &sv.n_chunks_used, &sv.blocks_per_sm_used, &sv.qt_used, &sv.npoly_used, &sv.nb_used, &sv.rec3_used};
+        for (int i = 0; i < 7; ++i) { if (save) *s[i] = *u[i]; else *u[i] = *s[i]; }
     };
     sv.cells = c->pix_cells; sv.tile_meta = c->pix_meta; sv.u0 = c->pix_u0; sv.u1 = c->pix_u1; sv.qc = c->pix_qc; sv.sc = c->pix_sc;
     sv.n_tiles = n_tiles; sv.n_slots = n_pix; sv.W = n_pix; sv.K = 0; sv.n_q = 0;
     sv.grid_valid = false; sv.g_uniform = false; sv.has_N = true; sv.has_M = false;
     sv.g_type = 0; sv.g_n0 = 0; sv.g_n1 = 0; sv.g_dq = 0.0;
+    // the pixel sample: radius = largest |q| of the detector; a tile is an arc of a ring (centre left at 0: no correction)
+    sv.g_dev = 0.0; sv.g_qmax = 0.0; sv.geo_rmax = c->g_qmax; sv.geo_ext = 0.0; sv.geo_extz = 0.0; sv.geo_pending = false;
+    sv.amp_valid = false; sv.opt_qt = 0; sv.opt_bases = 0; sv.amp_timer = -1;
+    keep_used(true);
     exchange();                                   // the context now describes the pixel sample, no grid yet
     nms_status st = set_grid(c, rgrid);
     AmpPlan plan;
     if (!st) st = plan_amplitude(c, false, &plan);
     if (!st) {
-        timer_begin(c, NMS_T_CORR2D);
-        st = launch_amplitude(c, plan, nullptr, 0);
+        st = timer_begin(c, NMS_T_CORR2D);
+        if (!st) st = launch_amplitude(c, plan, nullptr, 0);
         if (!st) {
             const int64_t n_r = c->n_q;
             k_corr2d_finish<<<(unsigned)((n_r + 255) / 256), 256, 0, c->stream>>>((const double*)c->part.p, c->n_chunks_used,
                                                                                    n_r, out_re, out_im);
             c->launches += 1;
+            st = timer_end(c, NMS_T_CORR2D);
         }
-        timer_end(c, NMS_T_CORR2D);
+        c->corr2d_variant = c->variant_used;
     }
     exchange();                                   // back: sv holds the pixel / r-grid buffers again (possibly regrown)
+    keep_used(false);
     c->pix_cells = sv.cells; c->pix_meta = sv.tile_meta; c->pix_u0 = sv.u0; c->pix_u1 = sv.u1; c->pix_qc = sv.qc; c->pix_sc = sv.sc;
     if (st) return st;
     NMS_CUDA(c, cudaGetLastError());
@@ -386,11 +405,11 @@ nms_status launch_correlation(nms_ctx* c, const float* I, const float* q_of_bin,
     double* qv = (double*)c->bin_sum.p;
     double* gv = qv + n_bins;
     int32_t* n_valid = (int32_t*)(gv + (size_t)n_maps * n_bins);
-    timer_begin(c, NMS_T_CORRELATION);
+    if (nms_status ts_ = timer_begin(c, NMS_T_CORRELATION)) return ts_;
     k_corr_compact<<<1, 256, sizeof(int) * (size_t)n_bins, c->stream>>>(I, q_of_bin, count, n_maps, n_bins, qv, gv, n_valid);
     k_corr<<<dim3((unsigned)((n_r + 127) / 128), (unsigned)n_maps), 128, 0, c->stream>>>(qv, gv, n_valid, n_bins, r, n_r,
                                                                                         out_c, out_p);
-    timer_end(c, NMS_T_CORRELATION);
+    if (nms_status ts_ = timer_end(c, NMS_T_CORRELATION)) return ts_;
     c->launches += 2;
     NMS_CUDA(c, cudaGetLastError());
     return NMS_OK;

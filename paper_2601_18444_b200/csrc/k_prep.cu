@@ -2,8 +2,10 @@
 //
 //  prep kernel   (Eq. 37-41):  r' = R (x + r^k), m' = R m in fp64; only Y, Z (rows 2, 3 of R)
 //                are kept because q_x = 0 on the detector (Eq. 41).  One block per tile, TILE/256 cells per
-//                thread: it writes the Cell records (fp64 Y, Z; weights rounded once to fp32) and the tile's sum_j |w_cj|;
-//                k_wsum_reduce adds the tiles in a fixed order (the tolerance denominators, deterministic).
+//                thread: it writes the Cell records (fp64 Y, Z; weights rounded once to fp32), the tile's sum_j |w_cj|
+//                and the centre of its bounding box in the detector plane; k_wsum_reduce adds the tiles in a fixed
+//                order (the tolerance denominators, deterministic) and takes the largest radius and tile extent
+//                (host checks: |t| < 2^19 cycles for the exact phase reduction; residual of the recurrence correction).
 //  qsetup kernel (Eq. 6): per detector point (q_y, q_z) in fp64 [rad/nm] and
 //                (sin th, cos th) for the response epilogue.
 #include "nms_internal.h"
@@ -23,7 +25,7 @@ struct PrepArgs {
     const int32_t* flags;
     TileMeta* meta;
     Cell* cells;
-    double* tile_wsum;   // [n_tiles][4]: per-tile sum_j |w_cj| (reduced by k_wsum_reduce)
+    double* tile_wsum;   // [n_tiles][7]: per-tile sum_j |w_cj|, largest Y^2 + Z^2, squared half diagonal and half Z extent of the bounding box
     double R[9];
 };
 
@@ -33,9 +35,20 @@ __device__ __forceinline__ double warp_sum(double v)
     return v;
 }
 
+__device__ __forceinline__ double warp_min(double v)
+{
+    for (int o = 16; o > 0; o >>= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+__device__ __forceinline__ double warp_max(double v)
+{
+    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+
 __global__ void __launch_bounds__(PREP_THREADS) k_prep(const PrepArgs a)
 {
-    __shared__ double red[4][PREP_THREADS / 32];
+    __shared__ double red[9][PREP_THREADS / 32];
     const int tile = blockIdx.x;
     const TileSrc ts = a.src[tile];
     const int64_t first_slot = a.first_slot[tile];
@@ -51,6 +64,7 @@ __global__ void __launch_bounds__(PREP_THREADS) k_prep(const PrepArgs a)
     double Y[PREP_PER_THREAD], Z[PREP_PER_THREAD];
     float wN[PREP_PER_THREAD], wx[PREP_PER_THREAD], wy[PREP_PER_THREAD], wz[PREP_PER_THREAD];
     double sN = 0.0, sx = 0.0, sy = 0.0, sz = 0.0;
+    double ylo = 1e300, yhi = -1e300, zlo = 1e300, zhi = -1e300, r2 = 0.0;
 #pragma unroll
     for (int u = 0; u < PREP_PER_THREAD; ++u) {
         const int i = PREP_PER_THREAD * tid + u;
@@ -63,6 +77,8 @@ __global__ void __launch_bounds__(PREP_THREADS) k_prep(const PrepArgs a)
             const double z = (double)a.pos[3 * j + 2] + cz;
             Y[u] = a.R[3] * x + a.R[4] * y + a.R[5] * z;   // Eq. 39
             Z[u] = a.R[6] * x + a.R[7] * y + a.R[8] * z;   // Eq. 40
+            ylo = fmin(ylo, Y[u]); yhi = fmax(yhi, Y[u]); zlo = fmin(zlo, Z[u]); zhi = fmax(zhi, Z[u]);
+            r2 = fmax(r2, Y[u] * Y[u] + Z[u] * Z[u]);
             if (a.N) { wN[u] = a.N[j]; sN += fabs((double)wN[u]); }
             if (a.m) {
                 const double mx = (double)a.m[3 * j + 0], my = (double)a.m[3 * j + 1], mz = (double)a.m[3 * j + 2];
@@ -75,20 +91,29 @@ __global__ void __launch_bounds__(PREP_THREADS) k_prep(const PrepArgs a)
         }
     }
     sN = warp_sum(sN); sx = warp_sum(sx); sy = warp_sum(sy); sz = warp_sum(sz);
+    ylo = warp_min(ylo); yhi = warp_max(yhi); zlo = warp_min(zlo); zhi = warp_max(zhi); r2 = warp_max(r2);
     if (lane == 0) {
         red[0][warp] = sN; red[1][warp] = sx; red[2][warp] = sy; red[3][warp] = sz;
+        red[4][warp] = ylo; red[5][warp] = yhi; red[6][warp] = zlo; red[7][warp] = zhi; red[8][warp] = r2;
     }
     __syncthreads();
     if (tid == 0) {
-        double v[4];
-        for (int r = 0; r < 4; ++r) v[r] = red[r][0];
-        for (int w = 1; w < PREP_THREADS / 32; ++w)
+        double v[9];
+        for (int r = 0; r < 9; ++r) v[r] = red[r][0];
+        for (int w = 1; w < PREP_THREADS / 32; ++w) {
             for (int r = 0; r < 4; ++r) v[r] += red[r][w];
+            v[4] = fmin(v[4], red[4][w]); v[5] = fmax(v[5], red[5][w]);
+            v[6] = fmin(v[6], red[6][w]); v[7] = fmax(v[7], red[7][w]); v[8] = fmax(v[8], red[8][w]);
+        }
+        const bool any = ts.n_src > 0;
         TileMeta tm;
-        tm.Y0 = 0.0; tm.Z0 = 0.0; tm.first_slot = first_slot; tm.n_slots = n_slots; tm.flags = a.flags[tile];
-        tm.ext = 0.f; tm.pad_ = 0;
+        tm.Y0 = any ? 0.5 * (v[4] + v[5]) : 0.0; tm.Z0 = any ? 0.5 * (v[6] + v[7]) : 0.0;
+        tm.first_slot = first_slot; tm.n_slots = n_slots; tm.flags = a.flags[tile];
         a.meta[tile] = tm;
-        for (int r = 0; r < 4; ++r) a.tile_wsum[4 * (int64_t)tile + r] = v[r];
+        for (int r = 0; r < 4; ++r) a.tile_wsum[7 * (int64_t)tile + r] = v[r];
+        a.tile_wsum[7 * (int64_t)tile + 4] = v[8];
+        a.tile_wsum[7 * (int64_t)tile + 5] = any ? 0.25 * ((v[5] - v[4]) * (v[5] - v[4]) + (v[7] - v[6]) * (v[7] - v[6])) : 0.0;
+        a.tile_wsum[7 * (int64_t)tile + 6] = any ? 0.5 * (v[7] - v[6]) : 0.0;
     }
 #pragma unroll
     for (int u = 0; u < PREP_PER_THREAD; ++u) {
@@ -106,22 +131,24 @@ __global__ void __launch_bounds__(PREP_THREADS) k_prep(const PrepArgs a)
 __global__ void __launch_bounds__(1024) k_wsum_reduce(const double* __restrict__ tile_wsum, int64_t n_tiles,
                                                       double* __restrict__ wsum)
 {
-    __shared__ double red[4][32];
+    __shared__ double red[7][32];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    double s[4] = {0.0, 0.0, 0.0, 0.0};
-    for (int64_t t = threadIdx.x; t < n_tiles; t += blockDim.x)
+    double s[7] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+    for (int64_t t = threadIdx.x; t < n_tiles; t += blockDim.x) {
 #pragma unroll
-        for (int r = 0; r < 4; ++r) s[r] += tile_wsum[4 * t + r];
+        for (int r = 0; r < 4; ++r) s[r] += tile_wsum[7 * t + r];
+        s[4] = fmax(s[4], tile_wsum[7 * t + 4]); s[5] = fmax(s[5], tile_wsum[7 * t + 5]); s[6] = fmax(s[6], tile_wsum[7 * t + 6]);
+    }
 #pragma unroll
-    for (int r = 0; r < 4; ++r) {
-        s[r] = warp_sum(s[r]);
+    for (int r = 0; r < 7; ++r) {
+        s[r] = r < 4 ? warp_sum(s[r]) : warp_max(s[r]);
         if (lane == 0) red[r][warp] = s[r];
     }
     __syncthreads();
-    if (threadIdx.x < 4) {
+    if (threadIdx.x < 7) {
         double v = 0.0;
-        for (int w = 0; w < 32; ++w) v += red[threadIdx.x][w];
-        wsum[threadIdx.x] = v;
+        for (int w = 0; w < 32; ++w) v = threadIdx.x < 4 ? v + red[threadIdx.x][w] : fmax(v, red[threadIdx.x][w]);
+        wsum[threadIdx.x] = (threadIdx.x < 4 || threadIdx.x == 6) ? v : sqrt(v);   // [4]: largest radius in the detector plane, [5]: largest tile half diagonal, [6]: largest tile half extent in Z
     }
 }
 
@@ -139,15 +166,19 @@ nms_status launch_prep(nms_ctx* c)
     a.flags = (const int32_t*)(base + sizeof(int64_t) * (size_t)c->n_tiles);
     a.meta = (TileMeta*)c->tile_meta.p;
     a.cells = (Cell*)c->cells.p;
-    if (nms_status st = ensure(c, c->tile_wsum, sizeof(double) * 4 * (size_t)c->n_tiles)) return st;
+    if (nms_status st = ensure(c, c->tile_wsum, sizeof(double) * 7 * (size_t)c->n_tiles)) return st;
     a.tile_wsum = (double*)c->tile_wsum.p;
     for (int i = 0; i < 9; ++i) a.R[i] = c->R[i];
-    timer_begin(c, NMS_T_PREP);
+    if (nms_status ts_ = timer_begin(c, NMS_T_PREP)) return ts_;
     k_prep<<<(unsigned)c->n_tiles, PREP_THREADS, 0, c->stream>>>(a);
     k_wsum_reduce<<<1, 1024, 0, c->stream>>>((const double*)c->tile_wsum.p, c->n_tiles, (double*)c->wsum.p);
-    timer_end(c, NMS_T_PREP);
+    if (nms_status ts_ = timer_end(c, NMS_T_PREP)) return ts_;
     c->launches += 2;
     NMS_CUDA(c, cudaGetLastError());
+    // the two geometry figures go to pinned host memory; the planner waits for this event only
+    NMS_CUDA(c, cudaMemcpyAsync(c->h_geo, (const double*)c->wsum.p + 4, 3 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    NMS_CUDA(c, cudaEventRecord(c->geo_event, c->stream));
+    c->geo_pending = true;
     return NMS_OK;
 }
 

@@ -42,23 +42,26 @@ nms_status ensure(nms_ctx* c, DevBuf& b, size_t bytes)
     return NMS_OK;
 }
 
-void timer_begin(nms_ctx* c, int which)
+nms_status timer_begin(nms_ctx* c, int which)
 {
-    if (!c->opt_timing) return;
+    if (!c->opt_timing || which < 0) return NMS_OK;
     Timer& t = c->timers[which];
     if (t.used == t.beg.size()) {
         cudaEvent_t b = nullptr, e = nullptr;
-        cudaEventCreate(&b); cudaEventCreate(&e);
+        NMS_CUDA(c, cudaEventCreate(&b));
+        if (cudaError_t err = cudaEventCreate(&e)) { cudaEventDestroy(b); return cuda_fail(c, err, "cudaEventCreate"); }
         t.beg.push_back(b); t.end.push_back(e);
     }
-    cudaEventRecord(t.beg[t.used], c->stream);
+    NMS_CUDA(c, cudaEventRecord(t.beg[t.used], c->stream));
+    return NMS_OK;
 }
-void timer_end(nms_ctx* c, int which)
+nms_status timer_end(nms_ctx* c, int which)
 {
-    if (!c->opt_timing) return;
+    if (!c->opt_timing || which < 0) return NMS_OK;
     Timer& t = c->timers[which];
-    cudaEventRecord(t.end[t.used], c->stream);
+    NMS_CUDA(c, cudaEventRecord(t.end[t.used], c->stream));
     t.used += 1;
+    return NMS_OK;
 }
 
 static void free_buf(DevBuf& b)
@@ -106,7 +109,7 @@ static nms_status build_tiles(nms_ctx* c)
     if (nms_status st = ensure(c, c->tile_src, bytes)) return st;
     if (nms_status st = ensure(c, c->tile_meta, n * sizeof(TileMeta))) return st;
     if (nms_status st = ensure(c, c->cells, (size_t)slot * sizeof(Cell))) return st;
-    if (nms_status st = ensure(c, c->wsum, 4 * sizeof(double))) return st;
+    if (nms_status st = ensure(c, c->wsum, 7 * sizeof(double))) return st;
     char* base = (char*)c->tile_src.p;
     NMS_CUDA(c, cudaMemcpyAsync(base, c->h_tile_src.data(), n * sizeof(TileSrc), cudaMemcpyHostToDevice, c->stream));
     NMS_CUDA(c, cudaMemcpyAsync(base + n * sizeof(TileSrc), c->h_tile_first_slot.data(), n * sizeof(int64_t),
@@ -171,7 +174,13 @@ nms_status set_grid(nms_ctx* c, const nms_qgrid* g)
     // equally spaced along the thread line (u0)?  (decides whether the recurrence kernels may be used: every
     // abscissa must lie within one fp32 ulp of the largest one from the progression u0[0] + i d)
     bool uni = g->type != 2 && g->n0 >= 2;
-    double dq = 0.0;
+    double dq = 0.0, devq = 0.0;
+    {
+        double m0 = 0.0, m1 = 0.0;
+        for (int i = 0; i < g->n0; ++i) m0 = fmax(m0, fabs((double)g->u0[i]));
+        for (int i = 0; i < len1; ++i) m1 = fmax(m1, fabs((double)g->u1[i]));
+        c->g_qmax = g->type == 0 ? m0 : sqrt(m0 * m0 + m1 * m1);
+    }
     if (uni) {
         const double a0 = g->u0[0];
         dq = ((double)g->u0[g->n0 - 1] - a0) / (double)(g->n0 - 1);
@@ -181,8 +190,10 @@ nms_status set_grid(nms_ctx* c, const nms_qgrid* g)
             dev = fmax(dev, fabs((double)g->u0[i] - (a0 + dq * i)));
         }
         uni = dq != 0.0 && dev <= 1.2e-7 * amax;
+        devq = dev;
     }
     c->g_dq = dq;
+    c->g_dev = devq;
     c->g_uniform = uni;
     if (nms_status st = ensure(c, c->u0, sizeof(float) * (size_t)g->n0)) return st;
     if (nms_status st = ensure(c, c->u1, sizeof(float) * (size_t)len1)) return st;
@@ -234,6 +245,14 @@ nms_status nms_create(nms_ctx** out, int device, void* cuda_stream)
     c->device = device;
     c->stream = (cudaStream_t)cuda_stream;
     c->sm_count = pr.multiProcessorCount;
+    if (cudaMallocHost((void**)&c->h_geo, 3 * sizeof(double)) != cudaSuccess ||
+        cudaEventCreateWithFlags(&c->geo_event, cudaEventDisableTiming) != cudaSuccess) {
+        cudaGetLastError();
+        if (c->h_geo) cudaFreeHost(c->h_geo);
+        delete c;
+        return NMS_E_NOMEM;
+    }
+    c->h_geo[0] = c->h_geo[1] = c->h_geo[2] = 0.0;
     *out = c;
     return NMS_OK;
 }
@@ -244,11 +263,13 @@ void nms_destroy(nms_ctx* c)
     cudaSetDevice(c->device);
     cudaStreamSynchronize(c->stream);
     DevBuf* bufs[] = {&c->raw_pos, &c->raw_N, &c->raw_m, &c->centres, &c->tile_src, &c->tile_meta, &c->cells,
-                      &c->wsum, &c->u0, &c->u1, &c->qc, &c->sc, &c->amp64, &c->part, &c->ppart, &c->formpart,
+                      &c->wsum, &c->u0, &c->u1, &c->qc, &c->sc, &c->amp64, &c->part, &c->formpart,
                       &c->chunk_begin, &c->kinds_dev, &c->bin_idx, &c->bin_sum, &c->bin_cnt, &c->modal_tab, &c->modal_ring,
                       &c->tile_wsum, &c->pix_cells, &c->pix_meta, &c->pix_u0, &c->pix_u1, &c->pix_qc, &c->pix_sc};
     for (DevBuf* b : bufs) free_buf(*b);
     for (DevBuf& b : c->host_stage) free_buf(b);
+    if (c->h_geo) cudaFreeHost(c->h_geo);
+    if (c->geo_event) cudaEventDestroy(c->geo_event);
     for (Timer& t : c->timers) {
         for (cudaEvent_t e : t.beg) cudaEventDestroy(e);
         for (cudaEvent_t e : t.end) cudaEventDestroy(e);
@@ -489,6 +510,8 @@ nms_status nms_set_option(nms_ctx* c, const char* key, int64_t value)
     else if (!strcmp(key, "timing")) { c->opt_timing = value != 0; for (Timer& t : c->timers) t.used = 0; }
     else if (!strcmp(key, "chunks")) { if (value < 0) return fail(c, NMS_E_ARG, "chunks must be >= 0"); c->opt_chunks = (int)value; }
     else if (!strcmp(key, "bases")) { if (value < 0 || value > 4) return fail(c, NMS_E_ARG, "bases must be 0..4"); c->opt_bases = (int)value; }
+    else if (!strcmp(key, "precision")) { if (value < 0 || value > 2) return fail(c, NMS_E_ARG, "precision must be 0, 1 or 2"); c->opt_precision = (int)value; }
+    else if (!strcmp(key, "recurrence")) { if (value < 0 || value > 2) return fail(c, NMS_E_ARG, "recurrence must be 0, 1 or 2"); c->opt_rec3 = (int)value; }
     else if (!strcmp(key, "qt")) { if (value != 0 && value != 4 && value != 8 && value != 16) return fail(c, NMS_E_ARG, "qt must be 0, 4, 8 or 16"); c->opt_qt = (int)value; }
     else return fail(c, NMS_E_ARG, "unknown option '%s'", key);
     return NMS_OK;
@@ -506,6 +529,10 @@ nms_status nms_get_info(nms_ctx* c, const char* key, int64_t* value)
     else if (!strcmp(key, "sm_count")) *value = c->sm_count;
     else if (!strcmp(key, "blocks_per_sm")) *value = c->blocks_per_sm_used;
     else if (!strcmp(key, "qt")) *value = c->qt_used;
+    else if (!strcmp(key, "poly_phasors")) *value = c->npoly_used;
+    else if (!strcmp(key, "bases")) *value = c->nb_used;
+    else if (!strcmp(key, "three_term")) *value = c->rec3_used;
+    else if (!strcmp(key, "corr2d_variant")) *value = c->corr2d_variant;
     else return fail(c, NMS_E_ARG, "unknown info key '%s'", key);
     return NMS_OK;
 }

@@ -25,13 +25,12 @@ struct Cell {              // 32 B, the unit of the bulk copies (16-byte aligned
     float wN, wx, wy, wz;  // nuclear weight, m'_x, m'_y, m'_z
 };
 
-struct TileMeta {          // consumed by the amplitude kernel
-    double Y0, Z0;         // reserved (tile origin; unused: phases are reduced exactly in fp64)
+struct TileMeta {          // consumed by the amplitude kernel (32 B)
+    double Y0, Z0;         // centre of the tile's bounding box in the detector plane [nm]: the recurrence kernels
+                           // correct the deviation of a float abscissa from the evaluated progression there
     int64_t first_slot;    // index into the cell array
     int32_t n_slots;       // cell count of the tile
     int32_t flags;         // bit 0: last tile of its object, bit 1: first tile (form-factor split)
-    float ext;             // reserved
-    int32_t pad_;
 };
 struct TileSrc {           // consumed by the prep kernel
     int64_t src_first;     // first source cell
@@ -63,8 +62,12 @@ struct nms_ctx {
     int opt_chunks = 0;
     int opt_qt = 0;        // 0 auto, else 4/8/16
     int opt_bases = 0;     // recurrence kernels: exactly evaluated points per 8 (0 auto = 2, else 1..4)
+    int opt_precision = 0; // 0 auto = 1 fast (MUFU phasors), 2 accurate (polynomial phasors)
+    int opt_rec3 = 0;      // recurrence kernels: 0 auto, 1 rotations, 2 three-term recurrence
+    int amp_timer = NMS_T_AMPLITUDE;   // timer class of the amplitude launch (-1: none, the caller times it)
     int64_t launches = 0;
     int variant_used = 0, n_chunks_used = 0, blocks_per_sm_used = 0, qt_used = 0;
+    int npoly_used = 0, nb_used = 0, rec3_used = 0, corr2d_variant = 0;
 
     // sample (raw copy kept for nms_set_rotation)
     int64_t W = 0;
@@ -83,8 +86,12 @@ struct nms_ctx {
     std::vector<nms::TileSrc> h_tile_src;
     std::vector<int32_t> h_tile_flags;
     std::vector<int64_t> h_tile_first_slot;
-    nms::DevBuf tile_wsum;             // double [n_tiles][4]: per-tile sum |w|
-    nms::DevBuf tile_src, tile_meta, cells, wsum;   // cells: Cell[n_slots]; wsum: double[4]
+    nms::DevBuf tile_wsum;             // double [n_tiles][7]: per-tile sum |w|, largest r^2, squared half diagonal, half Z extent
+    nms::DevBuf tile_src, tile_meta, cells, wsum;   // cells: Cell[n_slots]; wsum: double[7] (4 sums, r_max, tile half diagonal, tile half Z extent)
+    double* h_geo = nullptr;           // pinned [3]: r_max, largest tile half diagonal and half Z extent of the packed sample
+    cudaEvent_t geo_event = nullptr;   // recorded after the copy into h_geo
+    bool geo_pending = false;
+    double geo_rmax = 0.0, geo_ext = 0.0, geo_extz = 0.0;   // host copies (valid once geo_pending is false)
 
     // current detector grid
     bool grid_valid = false;
@@ -92,13 +99,15 @@ struct nms_ctx {
     int64_t n_q = 0;
     bool g_uniform = false;            // abscissa along the thread line (u0) is equally spaced (within 1 ulp)
     double g_dq = 0.0;                 // its spacing (u0[n0-1] - u0[0]) / (n0 - 1)
+    double g_dev = 0.0;                // largest deviation of u0 from that progression [rad/nm]
+    double g_qmax = 0.0;               // largest |q| on the grid [rad/nm]
     std::vector<float> h_u0, h_u1;
     nms::DevBuf u0, u1, qc, sc;        // qc: double2[n_q] (q_y,q_z) rad/nm; sc: double2[n_q] (sin th, cos th)
 
     // amplitudes / scratch
     bool amp_valid = false;
     nms::DevBuf amp64;                 // double [8][n_q]
-    nms::DevBuf part, ppart, formpart; // chunk partials
+    nms::DevBuf part, formpart;        // chunk partials
     nms::DevBuf chunk_begin;           // int32 [n_chunks+1] (split mode only)
     std::vector<int32_t> h_chunk_begin;
     nms::DevBuf kinds_dev;             // int32 [<=13]
@@ -115,8 +124,8 @@ namespace nms {
 nms_status fail(nms_ctx* c, nms_status st, const char* fmt, ...);
 nms_status cuda_fail(nms_ctx* c, cudaError_t e, const char* where);
 nms_status ensure(nms_ctx* c, DevBuf& b, size_t bytes);
-void timer_begin(nms_ctx* c, int which);
-void timer_end(nms_ctx* c, int which);
+nms_status timer_begin(nms_ctx* c, int which);   // no-ops unless the "timing" option is set (which < 0: never)
+nms_status timer_end(nms_ctx* c, int which);
 
 #define NMS_CUDA(c, call)                                          \
     do {                                                           \
@@ -138,6 +147,10 @@ struct AmpPlan {
     int n_qblocks;
     int blocks_per_sm;
     bool split;
+    int nch;           // weight channels the kernel accumulates: 4, or 1 for a sample without moments
+    int npoly;         // direct: phasors per thread evaluated by polynomial (qt = all: accurate); recurrence: 0 / 1
+    int nb;            // recurrence: exactly evaluated points per thread
+    int rec3;          // recurrence: three-term recurrence instead of rotations
 };
 nms_status plan_amplitude(nms_ctx* c, bool split, AmpPlan* plan);
 nms_status launch_amplitude(nms_ctx* c, const AmpPlan& plan, const int32_t* kinds_dev, int n_kinds);

@@ -62,6 +62,7 @@ def assert_amplitudes(A_gpu, A_ref, wsum, label=""):
 
 
 NULL_LEVEL = 1e-9   # a signed map below this fraction of its parent's maximum is "null by symmetry"
+SIGNED = (KI["NM"], KI["CHI"])
 
 
 def parent_maps(oracle_mod, A, th, P=None, sN=1.0, sM=1.0, invV=1.0):
@@ -72,24 +73,19 @@ def parent_maps(oracle_mod, A, th, P=None, sN=1.0, sM=1.0, invV=1.0):
     return {KI["NM"]: M[0] + M[1], KI["CHI"]: M[2]}
 
 
-FP32_SIGNED_FLOOR = 1e-5   # x max(parent): floor of the signed kinds in the MUFU-phasor kernels (reading 16)
+def assert_cross_sections(M_gpu, M_ref, kinds, label="", ref_max=None, parents=None, parent_max=None, signed_misses=None):
+    """north_star, literally: relative error <= 1e-3 wherever |oracle| > 1e-6 of the map's own maximum, for every
+    kind, the signed ones (NM, CHI) included.
 
+    One clarification only (reading 16 (i)): a signed map that is null by symmetry (max|oracle| <= 1e-9 of
+    its parent half-sum NUC + PROJ resp. SF: both sides hold rounding noise, 'its maximum' has no meaning) must stay
+    below 1e-6 max(parent) on the GPU.  parents: kind -> parent map at the compared points (None = taken from the rows
+    of M_ref).  ref_max / parent_max: maxima taken over a larger map than the points compared (sampled comparisons).
 
-def assert_cross_sections(M_gpu, M_ref, kinds, label="", ref_max=None, parents=None, fp32=False, parent_max=None):
-    """north_star: relative error <= 1e-3 wherever |oracle| > 1e-6 of its maximum.
-
-    parents (kind -> parent map at the compared points; None = taken from the rows of M_ref): for the signed
-    difference kinds NM and CHI (reading 16),
-      * a map that is null by symmetry (max|oracle| <= 1e-9 max parent: both sides hold rounding noise
-        only, 'its maximum' has no meaning) must stay below the floor 1e-6 max(parent) on the GPU;
-      * fp32=True (the kernels that evaluate phasors with MUFU, absolute error 2^-21.4 per value): the
-        floor is the larger of 1e-6 of the map's own maximum and 1e-5 max(parent).  X = 2 Re/Im(a b*) of
-        two amplitudes with errors dA obeys |dX| <= 2 (|a| + |b|) dA; on lattice-aligned detector points
-        whole layers of cells share one phase and their phasor errors add coherently (measured on reduced
-        C5 at q = 3, theta = pi: dA = 1.5e-3 = 5e-8 sum|w|, |dX| = 0.5 at parent = 1.8e5), so below
-        ~1e-5 max(parent) the 1e-3 relative test asks for more than sin.approx delivers.  The exact fp64
-        kernel is held to the literal criterion.
-    ref_max / parent_max: maxima taken over a larger map than the points compared (sampled comparisons)."""
+    signed_misses: None = a miss of NM / CHI fails the test like any other.  A list = the fp32-accumulating kernels on
+    workloads where DESIGN.md section 7 states that the criterion is NOT guaranteed for the signed kinds: their misses
+    are appended as (label, kind, points tested, points failing, worst relative error) and the caller reports them with
+    `report_signed_misses` (the test then shows as xfailed, never as passed)."""
     kinds = list(kinds)
     if parents is None:   # derive the parents from the oracle rows themselves when they are there
         parents = {}
@@ -101,7 +97,6 @@ def assert_cross_sections(M_gpu, M_ref, kinds, label="", ref_max=None, parents=N
         ref = M_ref[i]
         got = M_gpu[i].astype(np.float64)
         mx = np.abs(ref).max() if ref_max is None else ref_max[i]
-        floor = XS_FLOOR * mx
         par = parents.get(k)
         if par is not None:
             pmax = np.abs(par).max() if parent_max is None else parent_max[k]
@@ -109,13 +104,22 @@ def assert_cross_sections(M_gpu, M_ref, kinds, label="", ref_max=None, parents=N
                 worst = np.abs(got - ref).max()
                 assert worst <= XS_FLOOR * pmax, f"{label}: null kind {ni.KINDS[k]}: |gpu| up to {worst:.3e} > 1e-6 x parent max {pmax:.3e}"
                 continue
-            if fp32:
-                floor = max(floor, FP32_SIGNED_FLOOR * pmax)
-        sel = np.abs(ref) > floor
+        sel = np.abs(ref) > XS_FLOOR * mx
         if not np.any(sel):
             continue
         rel = np.abs(got[sel] - ref[sel]) / np.abs(ref[sel])
+        if rel.max() > XS_RTOL and k in SIGNED and signed_misses is not None:
+            signed_misses.append((label, ni.KINDS[k], int(sel.sum()), int((rel > XS_RTOL).sum()), float(rel.max())))
+            continue
         assert rel.max() <= XS_RTOL, f"{label}: kind {ni.KINDS[k]}: max rel err {rel.max():.3e} at {sel.sum()} points"
+
+
+def report_signed_misses(misses):
+    """Every other assertion of the test held; the north-star criterion for NM / CHI did not hold everywhere: xfail with
+    the measured numbers (DESIGN.md section 7 says where the fp32 kernels cannot guarantee it and why)."""
+    if misses:
+        pytest.xfail("north_star criterion missed for signed kinds (fp32 accumulation, DESIGN.md section 7): " +
+                     "; ".join(f"{lab} {kind}: {bad} of {n} points above 1e-3, worst {w:.2e}" for lab, kind, n, bad, w in misses))
 
 
 def _oracle_maps(oracle_mod, wl, qy, qz, th, kinds, R=None):
@@ -143,27 +147,40 @@ def _run_full(nms, h, wl, kinds):
 # C1, C2 at full size, full maps; every kernel variant the grid admits
 # ---------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("name", ["C1", "C2"])
-@pytest.mark.parametrize("variant,qt,bases", [(0, 0, 0), (3, 0, 0), (1, 0, 0), (1, 4, 0), (1, 8, 0),
-                                               (2, 0, 0), (2, 0, 1), (2, 0, 2), (2, 0, 3), (2, 0, 4)])
-def test_full_config_maps(nms, ctx, oracle_mod, name, variant, qt, bases):
-    """variant 0 = automatic (these small problems run the exact fp64 kernel: strict north_star criteria),
-    3 = exact forced, 1 = the fp32-accumulating direct kernels, 2 = the line-recurrence kernels with
-    `bases` exactly evaluated points per 8 (reading 16 floor for NM and CHI in the fp32 kernels)."""
+@pytest.mark.parametrize("variant,qt,bases,rec,prec", [(0, 0, 0, 0, 0), (3, 0, 0, 0, 0), (1, 0, 0, 0, 0), (1, 4, 0, 0, 0),
+                                                        (1, 8, 0, 0, 0), (1, 0, 0, 0, 2), (1, 4, 0, 0, 2),
+                                                        (2, 0, 0, 0, 0), (2, 0, 1, 1, 0), (2, 0, 2, 1, 0), (2, 0, 2, 2, 0),
+                                                        (2, 0, 3, 1, 0), (2, 0, 4, 1, 0), (2, 0, 0, 0, 2), (2, 0, 2, 2, 2)])
+def test_full_config_maps(nms, ctx, oracle_mod, name, variant, qt, bases, rec, prec):
+    """variant 0 = automatic (these small problems run the exact fp64 kernel), 3 = exact forced: every kind held to
+    the north_star criterion.  1 = the fp32-accumulating direct kernels, 2 = the line-recurrence kernels with `bases`
+    exactly evaluated points per 8 by rotations (rec 1) or the three-term recurrence (rec 2), MUFU (prec 0) or
+    polynomial (prec 2) phasors: amplitudes and every kind to the same criterion; a miss of NM / CHI is reported as
+    xfail (C1 and C2 are below the size where the library itself would pick an fp32 kernel)."""
     wl = ni.make_config(name)
     kinds = list(ni.ALL_KINDS)
     _upload(nms, ctx, wl)
     nms.nms_set_option(ctx, "variant", variant)
     nms.nms_set_option(ctx, "qt", qt)
     nms.nms_set_option(ctx, "bases", bases)
+    nms.nms_set_option(ctx, "recurrence", rec)
+    nms.nms_set_option(ctx, "precision", prec)
     A_gpu, M_gpu = _run_full(nms, ctx, wl, kinds)
     qy, qz, th = oracle_mod.grid_points(wl.grid)
     A, wsum, M = _oracle_maps(oracle_mod, wl, qy, qz, th, kinds)
     np.testing.assert_allclose(nms.nms_get_weight_sums(ctx), wsum, rtol=1e-12)
     assert_amplitudes(A_gpu, A, wsum, name)
-    assert_cross_sections(M_gpu, M, kinds, name, fp32=(variant in (1, 2)))
+    misses = [] if variant in (1, 2) else None
+    assert_cross_sections(M_gpu, M, kinds, name, signed_misses=misses)
     used = nms.nms_get_info(ctx, "variant_used")
     polar = wl.grid.type == 0
     assert used == {0: 8, 3: 8, 1: 2 if polar else 4, 2: 3 if polar else 5}[variant]
+    if variant in (1, 2):
+        assert (nms.nms_get_info(ctx, "poly_phasors") != 0) == (prec == 2)
+    if variant == 2:
+        assert nms.nms_get_info(ctx, "bases") == (bases or 1)
+        assert nms.nms_get_info(ctx, "three_term") == (1 if rec == 2 or (rec == 0 and prec == 0) else 0)
+    report_signed_misses(misses)
 
 
 def test_c1_physics_on_gpu(nms, ctx):
@@ -184,22 +201,28 @@ def test_c1_physics_on_gpu(nms, ctx):
 # reduced C3, C4, C5 (same structure, several tiles and a ragged tail), full maps
 # ---------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("name", ["C3", "C4", "C5"])
-@pytest.mark.parametrize("variant", [0, 1, 2])
-def test_small_config_maps(nms, ctx, oracle_mod, name, variant):
+@pytest.mark.parametrize("variant,prec", [(0, 0), (1, 0), (2, 0), (1, 2), (2, 2)])
+def test_small_config_maps(nms, ctx, oracle_mod, name, variant, prec):
+    """Every kernel family on the reduced configs, all 13 kinds at the north_star criterion (variant 0 picks the exact
+    kernel at these sizes; a miss of NM / CHI by an fp32 kernel is reported as xfail)."""
     if name == "C3" and variant == 2:
         pytest.skip("C3's |q| is log-spaced: no line recurrence (NMS_E_UNSUPPORTED, see test_error_codes)")
     wl = ni.make_config(name, small=True)
     kinds = list(ni.ALL_KINDS)
     nms.nms_set_option(ctx, "variant", variant)
+    nms.nms_set_option(ctx, "precision", prec)
     qy, qz, th = oracle_mod.grid_points(wl.grid)
     rots = wl.rotations if wl.rotations is not None else [wl.R]
     _upload(nms, ctx, wl)
+    misses = [] if variant else None
     for R in rots:
         nms.nms_set_rotation(ctx, R)
         A_gpu, M_gpu = _run_full(nms, ctx, wl, kinds)
         A, wsum, M = _oracle_maps(oracle_mod, wl, qy, qz, th, kinds, R=R)
         assert_amplitudes(A_gpu, A, wsum, name)
-        assert_cross_sections(M_gpu, M, kinds, name, fp32=(variant in (1, 2)))
+        assert_cross_sections(M_gpu, M, kinds, name, signed_misses=misses)
+        assert (nms.nms_get_info(ctx, "variant_used") == 8) == (variant == 0)
+    report_signed_misses(misses)
 
 
 @pytest.mark.parametrize("gtype", [0, 1])
@@ -217,9 +240,7 @@ def test_recurrence_ragged_lines(nms, ctx, oracle_mod, gtype, n0):
         grid = ni.polar_grid(np.linspace(0.02, 1.7, n0) if n0 > 1 else np.array([0.5]), 37)
     else:
         grid = ni.cartesian_grid(np.linspace(-0.9, 1.1, n0) if n0 > 1 else np.array([0.3]), np.linspace(-1.0, 1.0, 37))
-    # a fully incoherent random sample: the signed kinds cross zero everywhere at the level of their parents,
-    # so only the amplitudes and the positive kinds are compared here (the index logic is what is under test)
-    kinds = [KI[k] for k in ("NUC", "MAG", "UNPOL", "PROJ", "SF")]
+    kinds = list(ni.ALL_KINDS)   # a fully incoherent random sample: the signed kinds cross zero all over the detector
     import torch
     nms.nms_set_sample(ctx, _t(pos), _t(N), _t(m), R)
     nms.nms_set_option(ctx, "variant", 2 if n0 > 1 else 1)
@@ -234,7 +255,9 @@ def test_recurrence_ragged_lines(nms, ctx, oracle_mod, gtype, n0):
     A, wsum = oracle_mod.amplitudes(pos, N, m, R, qy, qz, return_wsum=True)
     M = oracle_mod.response(A, th, kinds)
     assert_amplitudes(amp.cpu().numpy(), A, wsum, f"ragged n0={n0}")
-    assert_cross_sections(maps.cpu().numpy(), M, kinds, f"ragged n0={n0}", fp32=True)
+    misses = []
+    assert_cross_sections(maps.cpu().numpy(), M, kinds, f"ragged n0={n0}", signed_misses=misses)
+    report_signed_misses(misses)
 
 
 # ---------------------------------------------------------------------------------------------------
@@ -242,25 +265,28 @@ def test_recurrence_ragged_lines(nms, ctx, oracle_mod, gtype, n0):
 # variant): the full GPU map against the oracle on a seeded subset of detector points; maxima for the
 # floors are taken over the GPU's full map
 # ---------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("name,n_sample", [("C3", 96), ("C4", 96), ("C5", 64)])
+@pytest.mark.parametrize("name,n_sample", [("C3", 96), ("C4", 64), ("C5", 64)])
 def test_full_size_sampled(nms, ctx, oracle_mod, name, n_sample):
+    """All 13 kinds; C4: 6 of its 36 rotations, spread over the scan."""
     import torch
     wl = ni.make_config(name)
     kinds = list(ni.ALL_KINDS)
     qy, qz, th = oracle_mod.grid_points(wl.grid)
     idx = ni.q_subset(wl.grid.n_q, n_sample, 9000 + int(name[1]))
-    rots = wl.rotations[:2] if wl.rotations is not None else [wl.R]
+    rots = [wl.rotations[i] for i in (0, 7, 13, 20, 27, 35)] if wl.rotations is not None else [wl.R]
     _upload(nms, ctx, wl)
     nq = wl.grid.n_q
     amp = torch.empty((8, nq), dtype=torch.float32, device="cuda")
     maps = torch.empty((len(kinds), nq), dtype=torch.float32, device="cuda")
+    misses = []
     for R in rots:
         nms.nms_set_rotation(ctx, R)
         nms.nms_amplitudes(ctx, wl.grid, amp)
         nms.nms_response(ctx, kinds, maps)
         nms.nms_synchronize(ctx)
-        # an fp32-accumulating kernel: direct for C3 (log-spaced |q|), line recurrence for C4 and C5
+        # an fp32-accumulating kernel: direct for C3 (log-spaced |q|), three-term line recurrence for C4 and C5
         assert nms.nms_get_info(ctx, "variant_used") == {"C3": 2, "C4": 5, "C5": 3}[name]
+        assert nms.nms_get_info(ctx, "poly_phasors") == 0
         A_gpu, M_gpu = amp.cpu().numpy(), maps.cpu().numpy()
         A, wsum = oracle_mod.amplitudes(wl.pos, wl.N, wl.m, R, qy[idx], qz[idx], offsets=wl.offsets,
                                         centres=wl.centres, return_wsum=True)
@@ -272,7 +298,100 @@ def test_full_size_sampled(nms, ctx, oracle_mod, name, n_sample):
         pmax = {KI["NM"]: full_max[kinds.index(KI["NUC"])] + full_max[kinds.index(KI["PROJ"])],
                 KI["CHI"]: full_max[kinds.index(KI["SF"])]}
         assert_cross_sections(M_gpu[:, idx], M, kinds, name, ref_max=full_max, parents=par, parent_max=pmax,
-                              fp32=True)
+                              signed_misses=misses)
+    report_signed_misses(misses)
+
+
+def test_c5_full_map_end_to_end(nms, ctx, oracle_mod):
+    """C5 at full size through the call sequence bench.py times (nms_compute, ring average, c(r), p(r)) against the
+    FULL fp64 map of the oracle (exact x-collapse, tests/c5_reference.py): amplitudes-free comparison of all 13 maps at
+    every one of the 262 144 detector points, the 512-ring I(q) (Eq. 30) and c(r), p(r) at 1024 r (Eq. 34-35
+    L205-L207).  The oracle side takes 1-3 minutes on the box's cores."""
+    import torch
+    import c5_reference
+    wl = ni.make_config("C5")
+    kinds = wl.kinds
+    A, wsum, th = c5_reference.full_reference(oracle_mod, wl)
+    M = oracle_mod.response(A, th, kinds, P=wl.P)
+    _upload(nms, ctx, wl)
+    nq, nb, nr, nk = wl.grid.n_q, wl.n_bins, len(wl.r), len(kinds)
+    f32 = dict(dtype=torch.float32, device="cuda")
+    maps, I, qb = torch.empty((nk, nq), **f32), torch.empty((nk, nb), **f32), torch.empty(nb, **f32)
+    cnt = torch.empty(nb, dtype=torch.int32, device="cuda")
+    c, p = torch.empty((nk, nr), **f32), torch.empty((nk, nr), **f32)
+    amp = torch.empty((8, nq), **f32)
+    nms.nms_compute(ctx, wl.grid, kinds, maps)
+    nms.nms_azimuthal_average(ctx, maps, nk, nb, wl.q_lo, wl.q_hi, I, qb, cnt)
+    nms.nms_correlation(ctx, I, qb, cnt, nk, nb, _t(wl.r), c, p)
+    nms.nms_amplitudes(ctx, wl.grid, amp)
+    nms.nms_synchronize(ctx)
+    assert nms.nms_get_info(ctx, "variant_used") == 3
+    np.testing.assert_allclose(nms.nms_get_weight_sums(ctx), wsum, rtol=1e-12)
+    assert_amplitudes(amp.cpu().numpy(), A, wsum, "C5 full map")
+    misses = []
+    assert_cross_sections(maps.cpu().numpy(), M, kinds, "C5 full map", signed_misses=misses)
+    # 1-D outputs.  north_star states a criterion for the 2-D cross sections only; what it implies for a ring mean and
+    # for its Fourier-Bessel transform follows by the triangle inequality (DESIGN.md section 7): maps within 1e-3
+    # relative above 1e-6 of their maximum give |dI(q_i)| <= 1e-3 (mean_j |f(q_i, th_j)| + 1e-6 max|f|), and
+    # |dc(r)| <= (1 / 2 pi^2) sum_i wq_i q_i^2 |j0(q_i r)| tol_I(q_i), |dp| = r^2 |dc|.  (A relative criterion on I, c, p
+    # themselves is meaningless where they vanish: the ring mean of the chiral map is zero by symmetry, L183, and
+    # c(r) of every kind oscillates about zero at large r.)  Valid for all kinds, signed ones included.
+    n0, n1 = wl.grid.n0, wl.grid.n1
+    I_ref = oracle_mod.azimuthal_polar(M, n0, n1)
+    assert np.array_equal(cnt.cpu().numpy(), np.full(nb, n1, dtype=np.int32))
+    tol_I = 1e-3 * (np.abs(M).reshape(nk, n0, n1).mean(axis=2) + 1e-6 * np.abs(M).max(axis=1)[:, None])
+    dI = np.abs(I.cpu().numpy().astype(np.float64) - I_ref)
+    assert np.all(dI <= tol_I), f"C5 I(q): worst |dI| / tol = {(dI / tol_I).max():.3f}"
+    q = wl.grid.u0.astype(np.float64)
+    r = wl.r.astype(np.float64)
+    wq = np.empty(n0)
+    wq[0], wq[-1] = 0.5 * (q[1] - q[0]), 0.5 * (q[-1] - q[-2])
+    wq[1:-1] = 0.5 * (q[2:] - q[:-2])
+    x = q[None, :] * r[:, None]
+    j0 = np.where(np.abs(x) < 1e-4, 1.0 - x * x / 6.0, np.sin(x) / np.where(x == 0.0, 1.0, x))
+    tol_c = (tol_I * (wq * q * q)[None, :]) @ np.abs(j0).T / (2.0 * np.pi ** 2)          # [nk, nr]
+    c_ref, p_ref = oracle_mod.correlation(I_ref, q, wl.r)
+    dc = np.abs(c.cpu().numpy().astype(np.float64) - c_ref)
+    dp = np.abs(p.cpu().numpy().astype(np.float64) - p_ref)
+    assert np.all(dc <= tol_c + 1e-7 * np.abs(c_ref)), f"C5 c(r): worst |dc| / tol = {(dc / tol_c).max():.3f}"
+    assert np.all(dp <= tol_c * r[None, :] ** 2 + 1e-7 * np.abs(p_ref)), "C5 p(r)"
+    # for the record: how close the 1-D outputs actually are, relative to their own maxima
+    print("C5 1-D outputs: max |dI| / max|I| per kind", (dI.max(axis=1) / np.abs(I_ref).max(axis=1)).max(),
+          "max |dc| / max|c|", (dc.max(axis=1) / np.abs(c_ref).max(axis=1)).max(),
+          "worst |dI| / tol", (dI / tol_I).max(), "worst |dc| / tol", (dc / tol_c).max())
+    report_signed_misses(misses)
+
+
+@pytest.mark.parametrize("chunks", [0, 7])
+def test_c3_full_size_split_sampled(nms, ctx, oracle_mod, chunks):
+    """Full C3 (K = 1000 objects of 4224 cells) through nms_form_factor_split, the call bench.py times: total AND form
+    (Eq. 49-50) of the config's four kinds against oracle.form_factor_split on a seeded subset of detector
+    points; automatic chunking (object-boundary table) and a forced 7-chunk split."""
+    import torch
+    wl = ni.make_config("C3")
+    kinds = wl.kinds
+    qy, qz, th = oracle_mod.grid_points(wl.grid)
+    idx = ni.q_subset(wl.grid.n_q, 64, 9003)
+    tot_ref, form_ref = oracle_mod.form_factor_split(wl.pos, wl.N, wl.m, wl.offsets, kinds, qy[idx], qz[idx], th[idx], R=wl.R,
+                                                     centres=wl.centres, P=wl.P)
+    _upload(nms, ctx, wl)
+    nms.nms_set_option(ctx, "chunks", chunks)
+    tot = torch.empty((len(kinds), wl.grid.n_q), dtype=torch.float32, device="cuda")
+    form = torch.empty_like(tot)
+    nms.nms_form_factor_split(ctx, wl.grid, kinds, tot, form)
+    nms.nms_synchronize(ctx)
+    assert nms.nms_get_info(ctx, "variant_used") == 2            # the fp32 direct kernel, per-particle instantiation
+    if chunks:
+        assert nms.nms_get_info(ctx, "n_chunks") == chunks
+    t, f = tot.cpu().numpy(), form.cpu().numpy()
+    assert_cross_sections(t[:, idx], tot_ref, kinds, "C3 split total", ref_max=np.abs(t.astype(np.float64)).max(axis=1))
+    assert_cross_sections(f[:, idx], form_ref, kinds, "C3 split form", ref_max=np.abs(f.astype(np.float64)).max(axis=1))
+    # the ordinary path gives the same total
+    maps = torch.empty_like(tot)
+    nms.nms_compute(ctx, wl.grid, kinds, maps)
+    nms.nms_synchronize(ctx)
+    assert_cross_sections(maps.cpu().numpy()[:, idx], tot_ref, kinds, "C3 ordinary total",
+                          ref_max=np.abs(t.astype(np.float64)).max(axis=1))
 
 
 def test_form_factor_split_small(nms, ctx, oracle_mod):
@@ -285,19 +404,29 @@ def test_form_factor_split_small(nms, ctx, oracle_mod):
         qy, qz, th = oracle_mod.grid_points(wl.grid)
         tot_ref, form_ref = oracle_mod.form_factor_split(wl.pos, wl.N, wl.m, wl.offsets, kinds, qy, qz, th, R=wl.R,
                                                          centres=wl.centres, P=wl.P)
-        for chunks in (0, 1, 3):
-            nms.nms_set_option(ctx, "chunks", chunks)
-            tot = torch.empty((len(kinds), wl.grid.n_q), dtype=torch.float32, device="cuda")
-            form = torch.empty_like(tot)
-            nms.nms_form_factor_split(ctx, wl.grid, kinds, tot, form)
+        misses = []
+        for variant, prec in ((0, 0), (1, 0), (1, 2)):   # exact kernel (automatic at this size), fp32 direct kernel, MUFU / polynomial
+            nms.nms_set_option(ctx, "variant", variant)
+            nms.nms_set_option(ctx, "precision", prec)
+            for chunks in (0, 1, 3):
+                nms.nms_set_option(ctx, "chunks", chunks)
+                tot = torch.empty((len(kinds), wl.grid.n_q), dtype=torch.float32, device="cuda")
+                form = torch.empty_like(tot)
+                nms.nms_form_factor_split(ctx, wl.grid, kinds, tot, form)
+                nms.nms_synchronize(ctx)
+                assert nms.nms_get_info(ctx, "variant_used") == (2 if variant else 8)
+                sm = misses if variant else None
+                assert_cross_sections(tot.cpu().numpy(), tot_ref, kinds, f"split total v{variant}", signed_misses=sm)
+                assert_cross_sections(form.cpu().numpy(), form_ref, kinds, f"split form v{variant}", signed_misses=sm)
+            nms.nms_set_option(ctx, "chunks", 0)
+            # the ordinary path gives the same total
+            maps = torch.empty_like(tot)
+            nms.nms_compute(ctx, wl.grid, kinds, maps)
             nms.nms_synchronize(ctx)
-            assert_cross_sections(tot.cpu().numpy(), tot_ref, kinds, "split total")
-            assert_cross_sections(form.cpu().numpy(), form_ref, kinds, "split form")
-        # the ordinary path gives the same total
-        maps = torch.empty_like(tot)
-        nms.nms_compute(ctx, wl.grid, kinds, maps)
-        nms.nms_synchronize(ctx)
-        assert_cross_sections(maps.cpu().numpy(), tot_ref, kinds, "ordinary total")
+            assert_cross_sections(maps.cpu().numpy(), tot_ref, kinds, "ordinary total", signed_misses=sm)
+        nms.nms_set_option(ctx, "variant", 0)
+        nms.nms_set_option(ctx, "precision", 0)
+    report_signed_misses(misses)
 
 
 def test_form_factor_split_uneven_objects(nms, ctx, oracle_mod):
@@ -320,10 +449,16 @@ def test_form_factor_split_uneven_objects(nms, ctx, oracle_mod):
     tot_ref, form_ref = oracle_mod.form_factor_split(pos, N, m, offsets, kinds, qy, qz, th, R=R, centres=cen)
     tot = torch.empty((len(kinds), grid.n_q), dtype=torch.float32, device="cuda")
     form = torch.empty_like(tot)
-    nms.nms_form_factor_split(ctx, grid, kinds, tot, form)
-    nms.nms_synchronize(ctx)
-    assert_cross_sections(tot.cpu().numpy(), tot_ref, kinds, "uneven total")
-    assert_cross_sections(form.cpu().numpy(), form_ref, kinds, "uneven form")
+    misses = []
+    for variant in (0, 1):                                   # exact kernel, then the fp32 per-particle kernel
+        nms.nms_set_option(ctx, "variant", variant)
+        nms.nms_form_factor_split(ctx, grid, kinds, tot, form)
+        nms.nms_synchronize(ctx)
+        assert nms.nms_get_info(ctx, "variant_used") == (2 if variant else 8)
+        sm = misses if variant else None
+        assert_cross_sections(tot.cpu().numpy(), tot_ref, kinds, "uneven total", signed_misses=sm)
+        assert_cross_sections(form.cpu().numpy(), form_ref, kinds, "uneven form", signed_misses=sm)
+    report_signed_misses(misses)
 
 
 # ---------------------------------------------------------------------------------------------------
@@ -470,9 +605,9 @@ def test_correlation_2d(nms, ctx, oracle_mod, variant):
         nms.nms_correlation_2d(ctx, maps[i], rgrid, re, im)
         nms.nms_synchronize(ctx)
         if variant == 0:
-            assert nms.nms_get_info(ctx, "variant_used") == 8          # small problem: exact kernel
+            assert nms.nms_get_info(ctx, "corr2d_variant") == 8        # small problem: exact kernel
         if variant == 2:
-            assert nms.nms_get_info(ctx, "variant_used") == 3          # rho is an arithmetic progression: recurrence
+            assert nms.nms_get_info(ctx, "corr2d_variant") == 3        # rho is an arithmetic progression: recurrence
         rre, rim = oracle_mod.correlation_2d(maps_h[i], wl.grid.u0, wl.grid.u1, rgrid.u0, rgrid.u1)
         sw = float((np.abs(maps_h[i].astype(np.float64)).reshape(n0, n1) * (q64 * wq)[:, None]).sum() * 2 * np.pi / n1)
         tol = (1e-5 if variant else 2e-7) * sw
@@ -565,19 +700,25 @@ def test_cross_spectra(nms, ctx, oracle_mod, name, small):
     with pytest.raises(nms.NmsError) as e:
         nms.nms_cross_spectra(ctx, GR, GI)
     assert e.value.status == nms.NMS_E_STATE                       # no amplitudes yet
+    worst = []
     for variant in (0, 1):
         nms.nms_set_option(ctx, "variant", variant)
         nms.nms_amplitudes(ctx, wl.grid, None)
         nms.nms_cross_spectra(ctx, GR, GI)
         nms.nms_synchronize(ctx)
-        floor = (1e-6 if variant == 0 else 1e-5) * gmax            # reading 16: off-diagonal components are signed
+        floor = 1e-6 * gmax                                        # of the largest |G|: the off-diagonal components are signed
         for got, ref in ((GR.cpu().numpy(), rGR), (GI.cpu().numpy(), rGI)):
             sel = np.abs(ref) > floor
-            assert np.all(np.abs(got[sel] - ref[sel]) <= 1e-3 * np.abs(ref[sel]))
-            assert np.all(np.abs(got - ref) <= 1e-3 * np.abs(ref) + 1e-3 * floor)
+            rel = np.abs(got[sel] - ref[sel]) / np.abs(ref[sel])
+            if variant == 0 or rel.max() <= 1e-3:
+                assert rel.max() <= 1e-3
+            else:
+                worst.append(f"{name} fp32 kernel: {(rel > 1e-3).sum()} of {sel.sum()} components above 1e-3, worst {rel.max():.2e}")
     with pytest.raises(nms.NmsError) as e:
         nms.nms_cross_spectra(ctx, None, None)
     assert e.value.status == nms.NMS_E_ARG
+    if worst:
+        pytest.xfail("; ".join(worst))
 
 
 def test_bench_line_sharded_step_matches_unsharded(nms):
@@ -674,15 +815,104 @@ def test_ragged_cell_counts(nms, ctx, oracle_mod, W):
     N = rng.uniform(-1, 1, size=W).astype(np.float32)
     m = rng.normal(size=(W, 3)).astype(np.float32)
     nms.nms_set_sample(ctx, _t(pos), _t(N), _t(m), None)
-    grid = ni.polar_grid(np.linspace(0.05, 2.0, 19), 37)              # 19 rings: ragged against QT = 4, 8, 16
+    grid = ni.polar_grid(np.linspace(0.05, 2.0, 19), 37)              # 19 rings: ragged against QT = 4, 8
     qy, qz, th = oracle_mod.grid_points(grid)
     A, wsum = oracle_mod.amplitudes(pos, N, m, None, qy, qz, return_wsum=True)
-    for qt in (4, 8):
+    amp = torch.empty((8, grid.n_q), dtype=torch.float32, device="cuda")
+    # partial tiles of 1 ... 9 cells and tails behind full tiles through the bulk-copy / mbarrier kernels: direct with
+    # 4 and 8 points per thread, MUFU and polynomial phasors, the line recurrence, and the exact kernel
+    for variant, qt, prec, used in ((1, 4, 0, 2), (1, 8, 0, 2), (1, 8, 2, 2), (2, 0, 0, 3), (2, 0, 2, 3), (0, 0, 0, 8)):
+        nms.nms_set_option(ctx, "variant", variant)
         nms.nms_set_option(ctx, "qt", qt)
-        amp = torch.empty((8, grid.n_q), dtype=torch.float32, device="cuda")
+        nms.nms_set_option(ctx, "precision", prec)
         nms.nms_amplitudes(ctx, grid, amp)
         nms.nms_synchronize(ctx)
-        assert_amplitudes(amp.cpu().numpy(), A, wsum, f"W={W} qt={qt}")
+        assert nms.nms_get_info(ctx, "variant_used") == used
+        if qt:
+            assert nms.nms_get_info(ctx, "qt") == qt
+        assert_amplitudes(amp.cpu().numpy(), A, wsum, f"W={W} variant={variant} qt={qt} precision={prec}")
+
+
+@pytest.mark.parametrize("variant,prec", [(0, 0), (1, 0), (1, 2)])
+def test_list_grid_against_oracle(nms, ctx, oracle_mod, variant, prec):
+    """A point-list detector with random non-zero q (MODE 2 kernel, 4 points per thread): amplitudes and all kinds."""
+    import torch
+    rng = np.random.Generator(np.random.Philox(606))
+    W, n = 2500, 1003                                                 # 1003 points: ragged against 128 threads x 4 points
+    pos = rng.uniform(-25, 25, size=(W, 3)).astype(np.float32)
+    N = rng.uniform(0.5, 1.5, size=W).astype(np.float32)
+    m = rng.normal(size=(W, 3)).astype(np.float32)
+    R = ni.rotation_alpha_beta(33.0, 71.0)
+    grid = ni.list_grid(rng.uniform(-1.5, 1.5, size=n), rng.uniform(-1.5, 1.5, size=n))
+    kinds = list(ni.ALL_KINDS)
+    nms.nms_set_sample(ctx, _t(pos), _t(N), _t(m), R)
+    nms.nms_set_option(ctx, "variant", variant)
+    nms.nms_set_option(ctx, "precision", prec)
+    amp = torch.empty((8, n), dtype=torch.float32, device="cuda")
+    maps = torch.empty((len(kinds), n), dtype=torch.float32, device="cuda")
+    nms.nms_amplitudes(ctx, grid, amp)
+    nms.nms_response(ctx, kinds, maps)
+    nms.nms_synchronize(ctx)
+    assert nms.nms_get_info(ctx, "variant_used") == (1 if variant else 8)
+    qy, qz, th = oracle_mod.grid_points(grid)
+    A, wsum = oracle_mod.amplitudes(pos, N, m, R, qy, qz, return_wsum=True)
+    M = oracle_mod.response(A, th, kinds)
+    assert_amplitudes(amp.cpu().numpy(), A, wsum, "list grid")
+    misses = [] if variant else None
+    assert_cross_sections(maps.cpu().numpy(), M, kinds, "list grid", signed_misses=misses)
+    report_signed_misses(misses)
+
+
+@pytest.mark.parametrize("gtype", [0, 1])
+def test_recurrence_far_from_the_origin(nms, ctx, oracle_mod, gtype):
+    """A sample translated by ~1e3 nm: the float abscissae of the line deviate from the evaluated progression by up to
+    one ulp(q), a phase of ulp(q) |r| ~ 1e-4 rad that the recurrence kernels correct at the tile centres; the exact
+    phase reduction is indifferent to the offset (|t| ~ 500 cycles << 2^19)."""
+    import torch
+    rng = np.random.Generator(np.random.Philox(919))
+    nx = 24
+    g = (np.arange(nx) - (nx - 1) / 2.0)
+    zz, yy, xx = np.meshgrid(g, g, g, indexing="ij")
+    pos = (np.stack([xx.ravel(), yy.ravel(), zz.ravel()], axis=1) + np.array([300.0, 900.0, -700.0])).astype(np.float32)
+    W = pos.shape[0]
+    N = np.ones(W, dtype=np.float32)
+    m = rng.normal(size=(W, 3)).astype(np.float32)
+    grid = ni.polar_grid(0.01 + np.arange(40) * (2.99 / 39), 48) if gtype == 0 else \
+        ni.cartesian_grid(np.linspace(-2.0, 2.1, 40), np.linspace(-2.0, 2.0, 33))
+    kinds = [KI[k] for k in ("NUC", "MAG", "UNPOL", "PROJ", "SF")]
+    nms.nms_set_sample(ctx, _t(pos), _t(N), _t(m), None)
+    qy, qz, th = oracle_mod.grid_points(grid)
+    A, wsum = oracle_mod.amplitudes(pos, N, m, None, qy, qz, return_wsum=True)
+    M = oracle_mod.response(A, th, kinds)
+    amp = torch.empty((8, grid.n_q), dtype=torch.float32, device="cuda")
+    maps = torch.empty((len(kinds), grid.n_q), dtype=torch.float32, device="cuda")
+    for rec in (1, 2):
+        nms.nms_set_option(ctx, "variant", 2)
+        nms.nms_set_option(ctx, "recurrence", rec)
+        nms.nms_amplitudes(ctx, grid, amp)
+        nms.nms_response(ctx, kinds, maps)
+        nms.nms_synchronize(ctx)
+        assert nms.nms_get_info(ctx, "variant_used") == (3 if gtype == 0 else 5)
+        assert_amplitudes(amp.cpu().numpy(), A, wsum, f"translated sample, recurrence {rec}")
+        assert_cross_sections(maps.cpu().numpy(), M, kinds, f"translated sample, recurrence {rec}")
+
+
+def test_phase_range_is_checked(nms, ctx):
+    """The adder-rounding phase reduction holds for |t| < 2^19 cycles: beyond it the fp32 kernels refuse
+    (NMS_E_UNSUPPORTED) instead of returning garbage; the exact kernel still runs."""
+    import torch
+    wl = ni.make_config("C1")
+    pos = (wl.pos.astype(np.float64) + np.array([0.0, 3.0e6, 0.0])).astype(np.float32)   # q r / 2 pi = 1.4e6 cycles
+    nms.nms_set_sample(ctx, _t(pos), _t(wl.N), _t(wl.m), None)
+    out = torch.empty((1, wl.grid.n_q), dtype=torch.float32, device="cuda")
+    nms.nms_set_option(ctx, "variant", 1)
+    with pytest.raises(nms.NmsError) as e:
+        nms.nms_compute(ctx, wl.grid, [0], out)
+    assert e.value.status == nms.NMS_E_UNSUPPORTED
+    nms.nms_set_option(ctx, "variant", 0)
+    nms.nms_compute(ctx, wl.grid, [0], out)
+    nms.nms_synchronize(ctx)
+    assert nms.nms_get_info(ctx, "variant_used") == 8
 
 
 def test_absent_channels(nms, ctx, oracle_mod):
@@ -761,4 +991,15 @@ def test_run_host_matches_device_path(nms, ctx):
     nms.nms_compute(ctx, wl.grid, kinds, maps)
     nms.nms_synchronize(ctx)
     assert np.array_equal(maps.cpu().numpy(), out_maps)
-    assert np.isfinite(out_I).all() and np.isfinite(out_c).all() and np.isfinite(out_p).all()
+    I = torch.empty((len(kinds), nb), dtype=torch.float32, device="cuda")
+    qb = torch.empty(nb, dtype=torch.float32, device="cuda")
+    cnt = torch.empty(nb, dtype=torch.int32, device="cuda")
+    c = torch.empty((len(kinds), nr), dtype=torch.float32, device="cuda")
+    p = torch.empty_like(c)
+    nms.nms_azimuthal_average(ctx, maps, len(kinds), nb, wl.q_lo, wl.q_hi, I, qb, cnt)
+    nms.nms_correlation(ctx, I, qb, cnt, len(kinds), nb, _t(wl.r), c, p)
+    nms.nms_synchronize(ctx)
+    # same kernels on the same maps: the histogram adds with fp64 atomics whose order is not fixed (last-bit differences)
+    np.testing.assert_allclose(out_I, I.cpu().numpy(), rtol=1e-6, atol=0)
+    np.testing.assert_allclose(out_c, c.cpu().numpy(), rtol=1e-5, atol=1e-7 * np.abs(out_c).max())
+    np.testing.assert_allclose(out_p, p.cpu().numpy(), rtol=1e-5, atol=1e-7 * np.abs(out_p).max())
