@@ -17,10 +17,10 @@ evaluated (no symmetry or merging tricks).  Rank 0 prints ONE JSON line.
  * cpu_baseline the fp64 oracle as it stands, timed on this box's host cores on a bounded sample
  * --impl reference   the oracle alone (this tier's reference arm), same metric and config
 
-N > 1 (torchrun): the path runs on one GPU (north_star); by default every rank runs an independent replica of
-the workload on its own GPU, no data-path collective; value = total pairs of all ranks /
-max-over-ranks time; scaling = weak.  --shard lines splits the detector lines of ONE workload over the ranks
-(cells replicated, all-gather of I(q) only); scaling = strong.
+N > 1: one process per GPU (under torchrun; `python bench.py --gpus N` alone starts the N ranks itself).  The detector
+lines of ONE workload are split over the ranks where the workload admits it (--shard auto / lines: cells replicated,
+all-gather of I(q) only; scaling = strong); otherwise, or with --shard replicas, every rank runs an independent
+replica (no data-path collective; value = total pairs of all ranks / max-over-ranks time; scaling = weak).
 """
 from __future__ import annotations
 
@@ -41,10 +41,20 @@ import nms_inputs as ni  # noqa: E402  (seeded input generators only; no arithme
 
 FP32_LANE_INSTR_PER_PAIR = 12      # 8 accumulate FFMA + 4 for the phasor
 LANES_PER_SM = 128
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE k_amp launch from the committed ncu --set full captures
-# (profiles/r1c_amp_kernels.md); null for workloads that were not captured.  The kernel is ALU-bound: the figure
-# only documents that DRAM traffic is irrelevant (C5: 4.5e-4 B per pair).
-NCU_DRAM_BYTES_PER_LAUNCH = {"C5": 1.632596e9 + 0.365705e9, "C3": 4.167948e9 + 7.983503e9}
+PREP_BYTES_PER_CELL = 60.0         # a-1: 28 B in (pos, N, m as float) + 32 B out (Cell record)
+
+
+def ncu_traffic(workload: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the workload's amplitude kernel, from the
+    committed summary of the `ncu --set full` captures (profiles/r2_traffic.json: workload -> kernel, bytes, commit);
+    None if the workload was not captured.  The kernel is ALU-bound: the figure documents that DRAM traffic is
+    irrelevant to the bound."""
+    path = os.path.join(ROOT, "profiles", "r2_traffic.json")
+    if not os.path.exists(path):
+        return None
+    with open(path) as f:
+        rec = json.load(f).get(workload)
+    return None if rec is None else float(rec["dram_bytes_read"]) + float(rec["dram_bytes_write"])
 
 
 def _env_int(name, default):
@@ -153,6 +163,7 @@ class Runner:
             self.h_c = torch.empty((nk, self.nr), dtype=torch.float32).pin_memory()
             self.h_p = torch.empty((nk, self.nr), dtype=torch.float32).pin_memory()
         self.rots = wl.rotations if wl.rotations is not None else [wl.R]
+        self.h_scan = torch.empty((len(self.rots), nk, nq), dtype=torch.float32).pin_memory() if len(self.rots) > 1 else None
         torch.cuda.synchronize(self.dev)
 
     # -- one pass of the hot path, raw arrays resident in HBM -------------------------------------------
@@ -195,12 +206,12 @@ class Runner:
                     self.h_c.copy_(self.c, non_blocking=True)
                     self.h_p.copy_(self.p, non_blocking=True)
 
-    # -- the same step from HOST buffers: H2D of the raw arrays and D2H of every result inside ------------
+    # -- the same step from HOST buffers: ONE C-ABI call, H2D of the raw arrays and D2H of every result inside ---------
     def step_host(self):
         nms, wl, h, torch = self.nms, self.wl, self.h, self.torch
-        if wl.split or len(self.rots) > 1 or self.shard is not None:
-            # nms_run_host covers one rotation without object structure; here the binding-level calls are
-            # used with explicit pinned copies (nms_set_sample accepts host pointers through UVA as well)
+        if self.shard is not None:
+            # line sharding under torchrun: the exchange step (all-gather of I(q)) sits between the passes, so the
+            # binding-level calls are used with explicit pinned copies (nms_set_sample accepts host pointers as well)
             self.d_pos.copy_(self.h_pos, non_blocking=True)
             if self.d_N is not None:
                 self.d_N.copy_(self.h_N, non_blocking=True)
@@ -210,7 +221,15 @@ class Runner:
                 self.d_cen.copy_(self.h_cen, non_blocking=True)
             self.step_device(d2h=True)
             torch.cuda.current_stream(self.dev).synchronize()
+        elif wl.split:
+            nms.nms_set_polarization(h, wl.P)
+            nms.nms_run_host_split(h, self.h_pos, self.h_N, self.h_m, wl.offsets, self.h_cen, wl.R, wl.grid, wl.kinds,
+                                   self.h_maps, self.h_form)
+        elif len(self.rots) > 1:
+            nms.nms_set_polarization(h, wl.P)
+            nms.nms_run_host_scan(h, self.h_pos, self.h_N, self.h_m, self.rots, wl.grid, wl.kinds, self.h_scan)
         else:
+            nms.nms_set_polarization(h, wl.P)
             nms.nms_run_host(h, self.h_pos, self.h_N, self.h_m, wl.R, wl.grid, wl.kinds, self.h_maps, self.nb, wl.q_lo,
                              wl.q_hi, self.h_I if self.nb else None, self.h_r if self.nr else None,
                              self.h_c if self.nr else None, self.h_p if self.nr else None)
@@ -291,6 +310,13 @@ def shard_lines(n0: int, world: int, rank: int):
     return i0, i0 + base + (1 if rank < extra else 0)
 
 
+def can_shard_lines(wl, world: int) -> bool:
+    """Line sharding covers polar and Cartesian detectors with at least one line per rank, except
+    |q| histograms on Cartesian detectors (bins straddle ranks)."""
+    g = wl.grid
+    return g.type != 2 and not (g.type == 1 and wl.n_bins) and g.n0 >= world
+
+
 def shard_workload(wl, world: int, rank: int):
     """This rank's part of a workload under line sharding: same sample, the detector lines [i0, i1)."""
     import copy
@@ -366,29 +392,26 @@ def oracle_sample(wl, n_sample):
 
 
 def parity_report(wl, maps_gpu, idx, M_ref):
-    """Worst relative deviation of the step's GPU maps from the oracle maps on the timed sample of detector points,
-    wherever |oracle| > 1e-6 of the GPU map's maximum (north_star criterion); the signed kinds NM and CHI are
-    reported separately above 1e-5 of their parents' maxima (reading 16)."""
+    """The step's GPU maps against the oracle maps on the timed sample of detector points, by the north_star criterion
+    taken literally: relative error wherever |oracle| > 1e-6 of the (GPU) map's own maximum, tolerance 1e-3, for every
+    kind.  The positive kinds and the signed difference kinds NM / CHI are reported separately; `signed_literal` says
+    how many of the tested points of the signed kinds miss the tolerance and by how much."""
     names = [ni.KINDS[k] for k in wl.kinds]
     fmax = np.abs(maps_gpu).max(axis=1)
-    def mx(name):
-        return fmax[names.index(name)] if name in names else 0.0
-    parent = {"NM": mx("NUC") + mx("PROJ"), "CHI": mx("SF")}
-    worst_pos, worst_signed = 0.0, 0.0
+    worst_pos, tested_pos, fail_pos = 0.0, 0, 0
+    worst_sig, tested_sig, fail_sig = 0.0, 0, 0
     for i, name in enumerate(names):
-        floor = 1e-6 * fmax[i]
-        if name in parent:
-            floor = max(floor, 1e-5 * parent[name])
-        sel = np.abs(M_ref[i]) > floor
+        sel = np.abs(M_ref[i]) > 1e-6 * fmax[i]
         if not sel.any():
             continue
-        rel = float((np.abs(maps_gpu[i][idx][sel] - M_ref[i][sel]) / np.abs(M_ref[i][sel])).max())
-        if name in parent:
-            worst_signed = max(worst_signed, rel)
+        rel = np.abs(maps_gpu[i][idx][sel] - M_ref[i][sel]) / np.abs(M_ref[i][sel])
+        if name in ("NM", "CHI"):
+            worst_sig, tested_sig, fail_sig = max(worst_sig, float(rel.max())), tested_sig + int(sel.sum()), fail_sig + int((rel > 1e-3).sum())
         else:
-            worst_pos = max(worst_pos, rel)
-    return {"points": int(len(idx)), "max_rel_err_positive_kinds": worst_pos, "max_rel_err_signed_kinds": worst_signed,
-            "tolerance": 1e-3}
+            worst_pos, tested_pos, fail_pos = max(worst_pos, float(rel.max())), tested_pos + int(sel.sum()), fail_pos + int((rel > 1e-3).sum())
+    return {"detector_points": int(len(idx)), "tolerance": 1e-3, "floor": "1e-6 of the map's own maximum",
+            "positive_kinds": {"points_tested": tested_pos, "points_failing": fail_pos, "worst_rel": worst_pos},
+            "signed_literal": {"points_tested": tested_sig, "points_failing": fail_sig, "worst_rel": worst_sig}}
 
 
 def time_oracle(wl, target_s=12.0, steps=1, warmup=0, keep=None):
@@ -445,13 +468,19 @@ WORKLOAD_TEXT = {
     "C3": "ensemble of 1000 spheres (R = 5 nm, 0.5 nm cells), total and form-factor outputs",
     "C4": "skyrmion-lattice film 512x512x8, rocking scan of 36 rotations about z",
     "C5": "micromagnetic block 256^3 with 5 % pores, all responses, I(q), c(r), p(r)",
-    "S4C": "context only: synthetic re-creation of the paper's Sec. IV C run (800 spheres x 4224 cells, 1000x1000 grid)",
 }
 
 
 def run_reference(args, rank):
     if rank != 0:
         return
+    if _env_int("WORLD_SIZE", 1) > 1:
+        # torchrun pins OMP_NUM_THREADS=1 for its workers; rank 0 alone runs the oracle, so give it the box's cores back
+        try:
+            import ctypes
+            ctypes.CDLL("libgomp.so.1").omp_set_num_threads(len(os.sched_getaffinity(0)))
+        except Exception:
+            pass
     wl = ni.make_config(args.workload)
     cb, ms = time_oracle(wl, target_s=args.oracle_seconds, steps=max(args.steps, 1), warmup=min(args.warmup, 1))
     line = {"impl": "reference", "metric": metric_name(), "value": cb["value"], "unit": "Gpair/s", "n_gpus": args.gpus,
@@ -489,21 +518,10 @@ def run_sweep(args):
                       "points": points}), flush=True)
 
 
-def run_cuda(args, rank, local_rank, world):
-    import torch
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device; the product has no CPU fallback (use --impl reference for the oracle)")
-    import paper_2601_18444_b200 as nms       # raises if libnms.so is missing and cannot be built
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-        torch.cuda.set_device(local_rank)
-        dist.init_process_group(backend="nccl", device_id=torch.device("cuda", local_rank))
+def measure(nms, torch, wl_full, args, steps, warmup, dist, rank, local_rank, world, sharded, headline):
+    """Time one workload: device-resident arm with the roofline of the amplitude kernel and, for the headline
+    workload, the end-to-end arm, the next rows, the oracle (cpu_baseline) and the parity of this very run."""
     dev = torch.device("cuda", local_rank)
-    torch.cuda.set_device(dev)
-
-    wl_full = ni.make_config(args.workload)
-    sharded = args.shard == "lines" and world > 1
     if sharded:
         wl, line0, line1 = shard_workload(wl_full, world, rank)
         run = Runner(nms, wl, local_rank, shard=(wl_full, world, rank, dist))
@@ -514,20 +532,20 @@ def run_cuda(args, rank, local_rank, world):
     sampler = ClockSampler(local_rank)
 
     # ---- device-resident arm -------------------------------------------------------------------------
-    for _ in range(args.warmup):
+    for _ in range(warmup):
         run.step_device()
     nms.nms_synchronize(h)
     launches0 = nms.nms_get_info(h, "launches")
     nms.nms_set_option(h, "timing", 1)                 # event pair around every kernel; resets the record
     sampler.start()
-    ms_total = _timed(torch, dev, run.step_device, args.steps, dist)
+    ms_total = _timed(torch, dev, run.step_device, steps, dist)
     sampler.stop()
     launches = nms.nms_get_info(h, "launches") - launches0
     kt = {name: nms.nms_kernel_time_total(h, idx) for name, idx in
           (("prep", nms.NMS_T_PREP), ("amplitude", nms.NMS_T_AMPLITUDE), ("epilogue", nms.NMS_T_EPILOGUE),
            ("azimuthal", nms.NMS_T_AZIMUTHAL), ("correlation", nms.NMS_T_CORRELATION))}
     nms.nms_set_option(h, "timing", 0)
-    ms_step = ms_total / args.steps
+    ms_step = ms_total / steps
     # replicas: every rank evaluates the whole workload (weak); line sharding: the ranks share ONE workload (strong)
     value = aggregate_rate(wl_full.pairs, 1 if sharded else world, ms_step)
 
@@ -542,7 +560,7 @@ def run_cuda(args, rank, local_rank, world):
     clocks = sampler.summary()
     roofline = {"bound": "alu", "kernel": "k_amp (a-2 amplitude sums)", "achieved": achieved, "peak": peak,
                 "unit": "T FP32 lane-instr/s (12 per pair)", "frac": achieved / peak,
-                "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(wl.name),
+                "traffic": ncu_traffic(wl.name),
                 "peak_source": f"{sm_count} SMs x 128 FP32 lanes x sm_max_mhz {peaks['sm_max_mhz']:.0f} ({peak_src})",
                 "gpair_s_kernel": pairs_per_launch / (amp_ms_per_launch * 1e-3) / 1e9,
                 "ms_per_launch": amp_ms_per_launch, "launches_timed": amp_n,
@@ -550,49 +568,96 @@ def run_cuda(args, rank, local_rank, world):
                 "frac_at_sampled_clock": (achieved / (sm_count * LANES_PER_SM * clocks["sm_mhz"] * 1e6 / 1e12))
                 if clocks.get("sm_mhz") else None,
                 "variant": nms.nms_get_info(h, "variant_used"), "qt": nms.nms_get_info(h, "qt"),
+                "bases": nms.nms_get_info(h, "bases"), "three_term": nms.nms_get_info(h, "three_term"),
+                "poly_phasors": nms.nms_get_info(h, "poly_phasors"),
                 "cell_chunks": nms.nms_get_info(h, "n_chunks"), "blocks_per_sm": nms.nms_get_info(h, "blocks_per_sm")}
-    passes = {}
-    hbm = peaks.get("hbm_gbs", 0.0)
-    nk, nq = len(wl.kinds), wl.grid.n_q
-    alg_bytes = {"prep": wl.W * 52.0,                                       # 28 B in, 24 B out per cell (a-1)
-                 "azimuthal": nk * nq * 4.0 + nk * max(wl.n_bins, 1) * 4.0,  # maps in, I(q) out (a-4)
-                 "correlation": nk * max(wl.n_bins, 1) * 4.0 + 2.0 * nk * max(run.nr, 1) * 4.0}   # a-5
-    for name in ("prep", "epilogue", "azimuthal", "correlation"):
-        t, n = kt[name]
-        if n:
-            passes[name] = {"ms_per_launch": t / n, "launches": n}
-            if name in alg_bytes:
-                gbs = alg_bytes[name] / (t / n * 1e-3) / 1e9
-                passes[name].update({"achieved_gbs": gbs, "frac_of_hbm_peak": gbs / hbm if hbm else None})
-
-    # ---- end-to-end arm: host buffers, copies inside the timed region --------------------------------
-    for _ in range(min(args.warmup, 2)):
-        run.step_host()
-    e2e_steps = max(1, min(args.steps, 3))
-    ms_e2e = _timed(torch, dev, run.step_host, e2e_steps, dist) / e2e_steps
-    h2d, d2h = run.bytes_per_step()
-    e2e = {"value": aggregate_rate(wl_full.pairs, 1 if sharded else world, ms_e2e), "unit": "Gpair/s", "ms_per_step": ms_e2e,
-           "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": e2e_steps}
-    next_rows = time_next_rows(nms, run, wl, torch, dev) if (wl.grid.type == 0 and not sharded) else None
-    maps_host = run.maps.cpu().numpy().astype(np.float64) if wl.n_rot == 1 else None   # the last step's maps
-    run.close()
-
-    cpu_baseline, parity = None, None
+    res = {"value": value, "ms_per_step": ms_step, "steps": steps, "warmup": warmup, "roofline": roofline,
+           "clocks": clocks, "gpu_launches": launches, "pairs_per_step": wl_full.pairs}
+    if headline:
+        passes = {}
+        hbm = peaks.get("hbm_gbs", 0.0)
+        nk, nq = len(wl.kinds), wl.grid.n_q
+        alg_bytes = {"prep": wl.W * PREP_BYTES_PER_CELL,                        # 28 B in, 32 B out per cell (a-1)
+                     "azimuthal": nk * nq * 4.0 + nk * max(wl.n_bins, 1) * 4.0,  # maps in, I(q) out (a-4)
+                     "correlation": nk * max(wl.n_bins, 1) * 4.0 + 2.0 * nk * max(run.nr, 1) * 4.0}   # a-5
+        for name in ("prep", "epilogue", "azimuthal", "correlation"):
+            t, n = kt[name]
+            if n:
+                passes[name] = {"ms_per_launch": t / n, "launches": n}
+                if name in alg_bytes:
+                    gbs = alg_bytes[name] / (t / n * 1e-3) / 1e9
+                    passes[name].update({"achieved_gbs": gbs, "frac_of_hbm_peak": gbs / hbm if hbm else None})
+        res["passes"] = passes
+        # ---- end-to-end arm: host buffers, copies inside the timed region ----------------------------
+        for _ in range(min(warmup, 3)):
+            run.step_host()
+        e2e_steps = max(1, min(steps, 10))
+        ms_e2e = _timed(torch, dev, run.step_host, e2e_steps, dist) / e2e_steps
+        h2d, d2h = run.bytes_per_step()
+        res["e2e"] = {"value": aggregate_rate(wl_full.pairs, 1 if sharded else world, ms_e2e), "unit": "Gpair/s",
+                      "ms_per_step": ms_e2e, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": e2e_steps}
+        res["next_rows"] = time_next_rows(nms, run, wl, torch, dev) if (wl.grid.type == 0 and not sharded) else None
+    # the maps of the FIRST rotation of one more (untimed) pass, for the parity object
+    maps_host = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        nms.nms_set_sample(h, run.d_pos, run.d_N, run.d_m, run.rots[0])
+        if wl.offsets is not None:
+            nms.nms_set_particles(h, wl.offsets, run.d_cen)
+        nms.nms_set_polarization(h, wl.P)
+        if wl.split:
+            nms.nms_form_factor_split(h, wl.grid, wl.kinds, run.maps, run.form)
+        else:
+            nms.nms_compute(h, wl.grid, wl.kinds, run.maps)
+        nms.nms_synchronize(h)
+        maps_host = run.maps.cpu().numpy().astype(np.float64)
+    run.close()
+    res["cpu_baseline"], res["parity"] = None, None
+    if maps_host is not None:
         keep = {}
-        cpu_baseline, _ = time_oracle(wl, target_s=args.oracle_seconds, keep=keep)
-        if maps_host is not None:                       # the oracle sample doubles as a parity check of this very run
-            parity = parity_report(wl, maps_host, keep["idx"], keep["M"])
+        res["cpu_baseline"], _ = time_oracle(wl, target_s=args.oracle_seconds if headline else min(args.oracle_seconds, 3.0), keep=keep)
+        res["parity"] = parity_report(wl, maps_host, keep["idx"], keep["M"])   # the oracle sample doubles as a parity check
+    return res
+
+
+def run_cuda(args, rank, local_rank, world):
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product has no CPU fallback (use --impl reference for the oracle)")
+    import paper_2601_18444_b200 as nms       # raises if libnms.so is missing and cannot be built
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        torch.cuda.set_device(local_rank)
+        dist.init_process_group(backend="nccl", device_id=torch.device("cuda", local_rank))
+    torch.cuda.set_device(torch.device("cuda", local_rank))
+
+    wl_full = ni.make_config(args.workload)
+    sharded = world > 1 and (args.shard == "lines" or (args.shard == "auto" and can_shard_lines(wl_full, world)))
+    res = measure(nms, torch, wl_full, args, args.steps, args.warmup, dist, rank, local_rank, world, sharded, True)
+    # the other two throughput configs of the north-star target (>= 60 % on C3-C5), timed OUTSIDE the headline region
+    configs = None
+    if world == 1 and not args.no_configs:
+        configs = {}
+        for name in ("C3", "C4", "C5"):
+            if name == args.workload:
+                continue
+            r = measure(nms, torch, ni.make_config(name), args, 3, 3, None, rank, local_rank, 1, False, False)
+            configs[name] = {"value": r["value"], "unit": "Gpair/s", "ms_per_step": r["ms_per_step"], "steps": r["steps"],
+                             "warmup": r["warmup"], "roofline_frac": r["roofline"]["frac"],
+                             "kernel_ms_per_launch": r["roofline"]["ms_per_launch"], "variant": r["roofline"]["variant"],
+                             "cell_chunks": r["roofline"]["cell_chunks"], "clocks": r["clocks"], "parity": r["parity"],
+                             "pairs_per_step": r["pairs_per_step"]}
 
     if rank == 0:
-        line = {"metric": metric_name(), "value": value, "unit": "Gpair/s", "n_gpus": world, "steps": args.steps,
-                "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
+        line = {"metric": metric_name(), "value": res["value"], "unit": "Gpair/s", "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": res["ms_per_step"], "higher_is_better": True,
                 "scaling": "strong" if sharded else "weak",
                 "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                 "config": workload_config(wl_full, {"parallelism": ("detector lines sharded over ranks, cells replicated, all-gather of I(q) only"
                                                                     if sharded else "replicas only") if world > 1 else "single GPU"}),
-                "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "passes": passes,
-                "next_rows": next_rows, "cpu_baseline": cpu_baseline, "parity": parity}
+                "clocks": res["clocks"], "e2e": res["e2e"], "gpu_launches": res["gpu_launches"], "roofline": res["roofline"],
+                "passes": res["passes"], "next_rows": res["next_rows"], "cpu_baseline": res["cpu_baseline"],
+                "parity": res["parity"], "configs": configs}
         print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()
@@ -603,21 +668,28 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="C5", choices=["C1", "C2", "C3", "C4", "C5", "S4C"])
+    ap.add_argument("--workload", default="C5", choices=["C1", "C2", "C3", "C4", "C5"])
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--oracle-seconds", type=float, default=12.0, help="CPU seconds per oracle step (bounded sample)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true",
                     help="context only: step time against cell count for the paper's Fig. 10 workload (one JSON line)")
-    ap.add_argument("--shard", default="replicas", choices=["replicas", "lines"],
-                    help="N > 1: independent replicas (default, weak scaling) or the detector lines of ONE workload "
-                         "shared by the ranks (strong scaling; DESIGN.md section 9)")
+    ap.add_argument("--shard", default="auto", choices=["auto", "replicas", "lines"],
+                    help="N > 1: the detector lines of ONE workload shared by the ranks (strong scaling; DESIGN.md "
+                         "section 9) or independent replicas (weak scaling); auto = lines where the workload admits it")
+    ap.add_argument("--no-configs", action="store_true", help="skip the C3 / C4 side measurements of the default line")
     args = ap.parse_args()
     rank, local_rank, world = _env_int("RANK", 0), _env_int("LOCAL_RANK", 0), _env_int("WORLD_SIZE", 1)
     if world != args.gpus and world > 1:
         raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}")
     if args.gpus > 1 and world == 1:
-        raise SystemExit("bench.py: for --gpus N > 1 launch with python -m torch.distributed.run --nproc-per-node N")
+        # not under torchrun: start the N ranks ourselves (one process per GPU) and become their launcher
+        import socket
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+        os.execv(sys.executable, [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+                                  "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:])
     if args.sweep:
         if rank == 0:
             run_sweep(args)

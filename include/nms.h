@@ -220,6 +220,20 @@ NMS_API nms_status nms_run_host(nms_ctx* ctx, const float* pos, const float* N, 
                         float* out_maps, int n_bins, double q_lo, double q_hi, float* out_I,
                         const float* r, int n_r, float* out_c, float* out_p);
 
+/* The same for a sample with object structure (a-6): copies pos/N/m [host][W], centres [host][K][3] (or NULL), runs
+ * nms_set_sample + nms_set_particles(offsets [host][K+1], K, centres) + nms_form_factor_split, copies out_total and
+ * out_form [host][n_kinds][n_q] (either may be NULL) back and synchronises.                                       */
+NMS_API nms_status nms_run_host_split(nms_ctx* ctx, const float* pos, const float* N, const float* m, int64_t W,
+                              const int64_t* offsets, int64_t K, const float* centres, const double* R,
+                              const nms_qgrid* grid, const nms_kind* kinds, int n_kinds, float* out_total,
+                              float* out_form);
+/* Rocking scan from HOST buffers (L7 "full rotational control"; config C4): the sample is copied once, then for each of
+ * the n_rot rotations R [host][n_rot][9] the prep pass and nms_compute run and the maps are copied to
+ * out_maps [host][n_rot][n_kinds][n_q]; synchronises before returning.                                             */
+NMS_API nms_status nms_run_host_scan(nms_ctx* ctx, const float* pos, const float* N, const float* m, int64_t W,
+                             const double* R, int n_rot, const nms_qgrid* grid, const nms_kind* kinds, int n_kinds,
+                             float* out_maps);
+
 /* ---- introspection / tuning --------------------------------------------------------------------- */
 
 /* sum_j |w_cj| of the rotated weights, c = N, m'x, m'y, m'z, into out [host][4] (the denominators of
@@ -227,17 +241,22 @@ NMS_API nms_status nms_run_host(nms_ctx* ctx, const float* pos, const float* N, 
 NMS_API nms_status nms_get_weight_sums(nms_ctx* ctx, double* out);
 
 /* Integer options.  "variant": 0 auto (exact fp64 kernel for W * n_q <= 2^30, else the line-recurrence
- * kernel where u0 is equally spaced, else the direct kernel), 1 force the direct (MUFU per pair) kernel,
- * 2 force the line-recurrence kernel (NMS_E_UNSUPPORTED at compute time if the detector is a point list or
- * u0 is not an arithmetic progression within one fp32 ulp), 3 force the exact fp64 kernel.  "bases": exactly
- * evaluated points per 8 in the recurrence kernel (0 auto = 2, else 1..4).  "timing": 1 records a CUDA
- * event pair around every kernel launch (and resets the record).  "chunks": 0 auto, else the number of cell
- * chunks.  "qt": 0 auto, else detector points per thread (4 or 8; 16 for the recurrence kernel on a sample
- * without moments).  Unknown keys: NMS_E_ARG.                                                            */
+ * kernel where u0 is equally spaced and the cell order is spatially coherent, else the direct kernel), 1 force the
+ * direct (one phasor per pair) kernel, 2 force the line-recurrence kernel (NMS_E_UNSUPPORTED at compute time if the
+ * detector is a point list or u0 is not an arithmetic progression within one fp32 ulp), 3 force the exact fp64
+ * kernel.  "precision": 0 / 1 MUFU phasors (sin.approx / cos.approx on the exactly reduced phase), 2 polynomial
+ * phasors on the FMA pipe, accurate to fp32 rounding (the selectable accurate variant of the fp32 kernels: 25-50 %
+ * slower).  "bases": exactly evaluated points per 8 in the recurrence kernel (0 auto = 1, else
+ * 1..4).  "recurrence": 0 auto, 1 complex rotations, 2 three-term recurrence (bases <= 2).  "timing": 1 records a
+ * CUDA event pair around every kernel launch (and resets the record).  "chunks": 0 auto, else the number of cell
+ * chunks.  "qt": 0 auto, else detector points per thread (4 or 8; 16 for the recurrence kernel on a sample without
+ * moments).  Unknown keys: NMS_E_ARG.  The fp32 kernels need q_max r_max / 2 pi < 2^19 cycles (NMS_E_UNSUPPORTED
+ * otherwise; the exact kernel has no such limit).                                                        */
 NMS_API nms_status nms_set_option(nms_ctx* ctx, const char* key, int64_t value);
 /* Read back integers: "launches" (kernels launched by this context so far), "variant_used" (1 list direct,
  * 2 polar direct, 4 cartesian direct, 3 polar recurrence, 5 cartesian recurrence, 8 exact fp64),
- * "n_chunks", "n_tiles", "n_slots", "sm_count", "blocks_per_sm", "qt".                              */
+ * "n_chunks", "n_tiles", "n_slots", "sm_count", "blocks_per_sm", "qt", "poly_phasors" (non-zero: polynomial phasors),
+ * "bases", "three_term", "corr2d_variant" (variant_used of the last nms_correlation_2d).             */
 NMS_API nms_status nms_get_info(nms_ctx* ctx, const char* key, int64_t* value);
 /* Device time in ms of the most recent launch of the given kernel class ("timing" must be 1);
  * synchronises on that kernel's end event.  NMS_E_STATE if it has not run.                       */

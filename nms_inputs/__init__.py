@@ -13,6 +13,6 @@ from .samples import (  # noqa: F401
     sphere_node_centred, sphere_cell_centred,
     Workload, KINDS, KIND_INDEX, ALL_KINDS,
     polar_grid, cartesian_grid, list_grid,
-    config_c1, config_c2, config_c3, config_c4, config_c5, config_sec4c, config_fig10, make_config,
+    config_c1, config_c2, config_c3, config_c4, config_c5, config_fig10, make_config,
     q_subset, uniform_sphere_sample, linear_vortex_sphere_sample, cuboid_lattice,
 )

@@ -259,16 +259,6 @@ def config_c3(K: int = 1000, n_q: int = 256, n_theta: int = 256, separate_centre
         offsets=(np.arange(K + 1, dtype=np.int64) * Nk), centres=cen, split=True)
 
 
-def config_sec4c(K: int = 800, n_q: int = 1000, n_theta: int = 1000) -> Workload:
-    """Context workload, not a BASELINE.json config: synthetic re-creation of the paper's Sec. IV C run (L682-L684:
-    800 spherical particles x 4224 cells, 1000 x 1000 (q, theta) grid, all outputs).  Same ensemble recipe as C3;
-    |q| linear in 0.01-3 nm^-1 (the paper does not state its grid); all 13 kinds, ring average, c(r), p(r)."""
-    w = config_c3(K=K, n_q=n_q, n_theta=n_theta)
-    q = 0.01 + 2.99 * np.arange(n_q, dtype=np.float64) / max(n_q - 1, 1)
-    return Workload(name="S4C", pos=w.pos, N=w.N, m=w.m, grid=polar_grid(q, n_theta), kinds=list(ALL_KINDS),
-                    n_bins=n_q, r=np.linspace(0.0, 30.0, 512).astype(np.float32))
-
-
 def config_fig10(K: int, n_q: int = 256, n_theta: int = 256) -> Workload:
     """Context workload, not a BASELINE.json config: synthetic re-creation of the paper's runtime experiment
     (Sec. IV D, Eq. 109): K identical spheres D = 40 nm on a node-centred a = 2 nm lattice (4169 cells
@@ -383,8 +373,6 @@ def make_config(name: str, small: bool = False) -> Workload:
         return config_c1()
     if name == "C2":
         return config_c2()
-    if name == "S4C":
-        return config_sec4c(K=6, n_q=40, n_theta=48) if small else config_sec4c()
     if name == "C3":
         return config_c3(K=6, n_q=40, n_theta=48) if small else config_c3()
     if name == "C4":

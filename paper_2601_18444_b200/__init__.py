@@ -34,7 +34,7 @@ EXPORTS = [
     "nms_set_rotation", "nms_set_polarization", "nms_set_scales", "nms_amplitudes", "nms_response", "nms_compute",
     "nms_azimuthal_average", "nms_correlation", "nms_form_factor_split", "nms_run_host", "nms_get_weight_sums",
     "nms_set_option", "nms_get_info", "nms_kernel_time_ms", "nms_kernel_time_total", "nms_modal_decomposition",
-    "nms_correlation_2d", "nms_cross_spectra",
+    "nms_correlation_2d", "nms_cross_spectra", "nms_run_host_split", "nms_run_host_scan",
 ]
 
 
@@ -226,6 +226,27 @@ def nms_run_host(ctx, pos, N, m, R, grid, kinds, out_maps, n_bins=0, q_lo=0.0, q
                                   C.byref(g), k, C.c_int(n), _hostbuf(out_maps), C.c_int(n_bins), C.c_double(q_lo),
                                   C.c_double(q_hi), _hostbuf(out_I), _hostbuf(r), C.c_int(n_r), _hostbuf(out_c),
                                   _hostbuf(out_p)))
+
+
+def nms_run_host_split(ctx, pos, N, m, offsets, centres, R, grid, kinds, out_total, out_form):
+    """nms_set_sample + nms_set_particles + nms_form_factor_split from HOST buffers; synchronises."""
+    g, keep = _grid_struct(grid)
+    k, n = _kinds(kinds)
+    Rh, Rp = _host(None if R is None else np.asarray(R, dtype=np.float64).reshape(9), np.float64)
+    off, offp = _host(offsets, np.int64)
+    _check(ctx, _lib.nms_run_host_split(ctx, _hostbuf(pos), _hostbuf(N), _hostbuf(m), C.c_int64(int(pos.shape[0])), offp,
+                                        C.c_int64(int(off.shape[0]) - 1), _hostbuf(centres), Rp, C.byref(g), k, C.c_int(n),
+                                        _hostbuf(out_total), _hostbuf(out_form)))
+
+
+def nms_run_host_scan(ctx, pos, N, m, rotations, grid, kinds, out_maps):
+    """Rocking scan from HOST buffers: rotations [n_rot][3][3]; out_maps [n_rot][n_kinds][n_q]; synchronises."""
+    g, keep = _grid_struct(grid)
+    k, n = _kinds(kinds)
+    Rs = np.ascontiguousarray(np.asarray(rotations, dtype=np.float64).reshape(-1, 9))
+    _check(ctx, _lib.nms_run_host_scan(ctx, _hostbuf(pos), _hostbuf(N), _hostbuf(m), C.c_int64(int(pos.shape[0])),
+                                       C.c_void_p(Rs.ctypes.data), C.c_int(int(Rs.shape[0])), C.byref(g), k, C.c_int(n),
+                                       _hostbuf(out_maps)))
 
 
 def nms_get_weight_sums(ctx) -> np.ndarray:

@@ -492,6 +492,43 @@ nms_status nms_run_host(nms_ctx* c, const float* pos, const float* N, const floa
     return NMS_OK;
 }
 
+nms_status nms_run_host_split(nms_ctx* c, const float* pos, const float* N, const float* m, int64_t W, const int64_t* offsets,
+                              int64_t K, const float* centres, const double* R, const nms_qgrid* grid, const nms_kind* kinds,
+                              int n_kinds, float* out_total, float* out_form)
+{
+    CHECK_CTX(c);
+    if (!grid || n_kinds <= 0 || (!out_total && !out_form)) return fail(c, NMS_E_ARG, "grid NULL, n_kinds <= 0 or no output");
+    if (nms_status st = set_sample_impl(c, pos, N, m, W, R)) return st;
+    if (nms_status st = nms_set_particles(c, offsets, K, centres)) return st;
+    const size_t bytes = sizeof(float) * (size_t)grid->n0 * grid->n1 * n_kinds;
+    DevBuf& d_tot = c->host_stage[0]; DevBuf& d_form = c->host_stage[7];
+    if (nms_status st = ensure(c, d_tot, bytes)) return st;
+    if (nms_status st = ensure(c, d_form, bytes)) return st;
+    if (nms_status st = nms_form_factor_split(c, grid, kinds, n_kinds, (float*)d_tot.p, (float*)d_form.p)) return st;
+    if (out_total) NMS_CUDA(c, cudaMemcpyAsync(out_total, d_tot.p, bytes, cudaMemcpyDeviceToHost, c->stream));
+    if (out_form) NMS_CUDA(c, cudaMemcpyAsync(out_form, d_form.p, bytes, cudaMemcpyDeviceToHost, c->stream));
+    NMS_CUDA(c, cudaStreamSynchronize(c->stream));
+    return NMS_OK;
+}
+
+nms_status nms_run_host_scan(nms_ctx* c, const float* pos, const float* N, const float* m, int64_t W, const double* R,
+                             int n_rot, const nms_qgrid* grid, const nms_kind* kinds, int n_kinds, float* out_maps)
+{
+    CHECK_CTX(c);
+    if (!grid || n_kinds <= 0 || n_rot <= 0 || !R || !out_maps) return fail(c, NMS_E_ARG, "NULL argument or non-positive count");
+    const size_t count = (size_t)grid->n0 * grid->n1 * n_kinds;
+    DevBuf& d_maps = c->host_stage[0];
+    if (nms_status st = ensure(c, d_maps, sizeof(float) * count * 2)) return st;      // two buffers: copy out while the next rotation runs
+    for (int i = 0; i < n_rot; ++i) {
+        if (nms_status st = (i == 0 ? set_sample_impl(c, pos, N, m, W, R) : nms_set_rotation(c, R + 9 * (size_t)i))) return st;
+        float* dst = (float*)d_maps.p + (size_t)(i & 1) * count;
+        if (nms_status st = nms_compute(c, grid, kinds, n_kinds, dst)) return st;
+        NMS_CUDA(c, cudaMemcpyAsync(out_maps + (size_t)i * count, dst, sizeof(float) * count, cudaMemcpyDeviceToHost, c->stream));
+    }
+    NMS_CUDA(c, cudaStreamSynchronize(c->stream));
+    return NMS_OK;
+}
+
 nms_status nms_get_weight_sums(nms_ctx* c, double* out)
 {
     CHECK_CTX(c);

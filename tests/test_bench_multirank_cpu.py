@@ -85,3 +85,27 @@ def test_reference_arm_other_ranks_exit_without_work():
                          capture_output=True, text=True, timeout=120, env=env, cwd=ROOT)
     assert out.returncode == 0, out.stderr[-2000:]
     assert out.stdout.strip() == ""
+
+
+def test_gpus_n_without_torchrun_starts_its_own_ranks():
+    """`python bench.py --gpus 2` outside torchrun re-executes itself under torch.distributed.run with 2 ranks on
+    127.0.0.1 (driven here through the oracle arm, which needs no GPU): exactly one JSON line, n_gpus = 2."""
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "LOCAL_RANK", "WORLD_SIZE", "MASTER_ADDR", "MASTER_PORT")}
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2", "--workload", "C1",
+                          "--oracle-seconds", "0.5", "--steps", "1", "--warmup", "0"],
+                         capture_output=True, text=True, timeout=300, env=env, cwd=ROOT)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [l for l in out.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["impl"] == "reference" and d["n_gpus"] == 2 and d["cpu_baseline"]["cores"] >= 1
+
+
+def test_auto_sharding_rule():
+    sys.path.insert(0, ROOT)
+    import bench
+    import nms_inputs as ni
+    assert bench.can_shard_lines(ni.make_config("C5", small=True), 8)         # polar rings
+    assert bench.can_shard_lines(ni.make_config("C4", small=True), 2)         # Cartesian rows, no histogram
+    assert not bench.can_shard_lines(ni.make_config("C2"), 2)                 # |q| histogram on a Cartesian detector
+    assert not bench.can_shard_lines(ni.make_config("C5", small=True), 64)    # more ranks than rings

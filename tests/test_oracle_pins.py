@@ -38,6 +38,30 @@ def test_dimer_closed_form(oracle_mod):
 
 
 # --------------------------------------------------------------------------- O2
+def test_cartesian_and_list_grid_axis_convention(oracle_mod):
+    """include/nms.h: a Cartesian grid has u0 = q_z [n0] (slow index) and u1 = q_y [n1] (fast index); a list grid
+    u0 = q_y, u1 = q_z; theta = atan2(q_y, q_z) from +z towards +y (Eq. 6).  Pinned with distinguishable axes: a
+    dimer along y only has |N~|^2 = 2 + 2 cos(q_y d), which must vary along u1 and not along u0."""
+    d = 3.0
+    pos = np.array([[0.0, -d / 2, 0.0], [0.0, d / 2, 0.0]], dtype=np.float32)
+    N = np.ones(2, dtype=np.float32)
+    qz = np.array([-0.7, 0.1, 0.4], dtype=np.float32)              # u0, n0 = 3
+    qy = np.array([-0.9, -0.2, 0.3, 0.8, 1.1], dtype=np.float32)   # u1, n1 = 5
+    grid = ni.cartesian_grid(qz, qy)
+    gy, gz, th = oracle_mod.grid_points(grid)
+    assert np.array_equal(gz.reshape(3, 5), np.repeat(qz.astype(np.float64)[:, None], 5, axis=1))
+    assert np.array_equal(gy.reshape(3, 5), np.repeat(qy.astype(np.float64)[None, :], 3, axis=0))
+    np.testing.assert_allclose(th, np.arctan2(gy, gz), rtol=0, atol=1e-15)
+    A = oracle_mod.amplitudes(pos, N, None, None, gy, gz)
+    F2 = (A[0] ** 2 + A[1] ** 2).reshape(3, 5)
+    np.testing.assert_allclose(F2, np.repeat((2 + 2 * np.cos(qy.astype(np.float64) * d))[None, :], 3, axis=0), rtol=1e-13)
+    assert np.ptp(F2, axis=0).max() < 1e-12 and np.ptp(F2, axis=1).min() > 0.1      # constant along u0, varying along u1
+    lst = ni.list_grid(qy[:3], qz)                                  # list: u0 = q_y, u1 = q_z
+    ly, lz, lth = oracle_mod.grid_points(lst)
+    assert np.array_equal(ly, qy[:3].astype(np.float64)) and np.array_equal(lz, qz.astype(np.float64))
+    np.testing.assert_allclose(lth, np.arctan2(ly, lz), rtol=0, atol=1e-15)
+
+
 def test_forward_amplitude_is_weight_sum(oracle_mod):
     """F(0) = sum w (north_star): at q = 0, A = (sum N, R sum m) with zero imaginary parts."""
     rng = np.random.default_rng(1)
