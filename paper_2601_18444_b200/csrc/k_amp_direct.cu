@@ -28,8 +28,9 @@ static amp_kernel_t pick_mode(int qt, bool split, int nch, int npoly)
     return nullptr;
 }
 
-amp_kernel_t amp_kernel_direct(int mode, int qt, bool split, int nch, int npoly)
+amp_kernel_t amp_kernel_direct(int mode, int qt, bool split, int nch, int npoly, bool uni)
 {
+    (void)uni;   // block-uniform abscissae were measured slower in the direct kernels (C3: 0.652 -> 0.618)
     switch (mode) {
     case 0: return pick_mode<0>(qt, split, nch, npoly);
     case 1: return pick_mode<1>(qt, split, nch, npoly);

@@ -58,11 +58,11 @@ __global__ void __launch_bounds__(AMP_THREADS) k_amp_f64(const AmpArgs a)
 static amp_kernel_t pick_kernel(const AmpPlan& p)
 {
     switch (p.variant) {
-    case 1: return amp_kernel_direct(2, p.qt, p.split, p.nch, p.npoly);
-    case 2: return amp_kernel_direct(0, p.qt, p.split, p.nch, p.npoly);
-    case 4: return amp_kernel_direct(1, p.qt, p.split, p.nch, p.npoly);
-    case 3: return amp_kernel_rec_polar(p.qt, p.nb, p.split, p.nch, p.npoly != 0, p.rec3 != 0);
-    case 5: return amp_kernel_rec_cart(p.qt, p.nb, p.split, p.nch, p.npoly != 0, p.rec3 != 0);
+    case 1: return amp_kernel_direct(2, p.qt, p.split, p.nch, p.npoly, false);
+    case 2: return amp_kernel_direct(0, p.qt, p.split, p.nch, p.npoly, p.uni);
+    case 4: return amp_kernel_direct(1, p.qt, p.split, p.nch, p.npoly, p.uni);
+    case 3: return amp_kernel_rec_polar(p.qt, p.nb, p.split, p.nch, p.npoly != 0, p.rec3 != 0, p.uni);
+    case 5: return amp_kernel_rec_cart(p.qt, p.nb, p.split, p.nch, p.npoly != 0, p.rec3 != 0, p.uni);
     default: return p.split ? (amp_kernel_t)k_amp_f64<true> : (amp_kernel_t)k_amp_f64<false>;
     }
 }
@@ -138,6 +138,7 @@ nms_status plan_amplitude(nms_ctx* c, bool split, AmpPlan* plan)
     } else if (p.variant != 8) {
         p.npoly = accurate ? p.qt : 0;
     }
+    p.uni = c->g_n1 % AMP_THREADS == 0 && c->opt_uniform != 1;
     amp_kernel_t kern = pick_kernel(p);
     if (!kern) return fail(c, NMS_E_ARG, "no amplitude kernel for variant %d qt %d bases %d polynomial %d three-term %d",
                            p.variant, p.qt, p.nb, p.npoly, p.rec3);

@@ -192,7 +192,9 @@ template <int QT, int NB> struct Seg {
 // NB = 0: direct evaluation of every pair (NPOLY of the QT phasors by polynomial, the others by MUFU);
 // NB > 0: line recurrence with NB exactly evaluated points per QT (NPOLY != 0: bases and step by polynomial),
 //         REC3 = 1: three-term recurrence instead of rotations.
-template <int MODE, int QT, bool SPLIT, int MINB, int NB, int NCH, int NPOLY, int REC3>
+// UNI: the launch guarantees n1 % 128 == 0, so a block lies inside ONE group of QT lines: the line abscissae are then
+//      block-uniform values (derived from blockIdx only), which frees the 2 QT registers a thread needs for them.
+template <int MODE, int QT, bool SPLIT, int MINB, int NB, int NCH, int NPOLY, int REC3, bool UNI = false>
 __global__ void __launch_bounds__(AMP_THREADS, MINB) k_amp(const AmpArgs a)
 {
     static_assert(NB == 0 || (MODE != 2 && NB <= QT), "the recurrence needs a line of equally spaced abscissae");
@@ -212,7 +214,15 @@ __global__ void __launch_bounds__(AMP_THREADS, MINB) k_amp(const AmpArgs a)
     int64_t slot = (int64_t)blockIdx.x * AMP_THREADS + tid;
     const bool valid = slot < n_slots_q;
     if (!valid) slot = 0;
-    const int grp = (int)(slot / a.n1), i1 = (int)(slot % a.n1);
+    int grp, i1;
+    if (UNI) {
+        const int bpg = a.n1 / AMP_THREADS;            // blocks per group of QT lines
+        grp = (int)blockIdx.x / bpg;
+        i1 = ((int)blockIdx.x % bpg) * AMP_THREADS + tid;
+    } else {
+        grp = (int)(slot / a.n1);
+        i1 = (int)(slot % a.n1);
+    }
     const int i0 = grp * QT;
     const int kmax = valid ? min(QT, a.n0 - i0) : 0;
     const int kclamp = max(min(QT, a.n0 - i0), 1);
@@ -224,14 +234,22 @@ __global__ void __launch_bounds__(AMP_THREADS, MINB) k_amp(const AmpArgs a)
 #pragma unroll
     for (int k = 0; k < QT; ++k) {
         const int kk = min(k, kclamp - 1);
-        if (MODE == 0) {
-            g[k] = (double)a.u0[i0 + kk] * INV_2PI;
-            h[k] = 0.0;
+        if (MODE == 0 || (MODE == 1 && UNI)) {
+            g[k] = (double)a.u0[i0 + kk] * INV_2PI;                          // |q|'_k, or q'_z,k of a Cartesian line
+            h[k] = MODE == 1 ? a.qc[flat0].x * INV_2PI : 0.0;                // q'_y
         } else {
             const double2 q = a.qc[flat0 + (int64_t)kk * a.n1];
             g[k] = q.y * INV_2PI;      // q'_z
             h[k] = q.x * INV_2PI;      // q'_y
         }
+    }
+    // keep the abscissae as opaque fp64 values: where registers are short the compiler otherwise re-derives them from
+    // the float grid inside the cell loop (F2F.F64.F32 + DMUL per point and iteration -- F2F runs on the XU pipe, the
+    // very pipe the direct kernels are bound by: measured 4.7 % of its capacity in the per-particle kernel)
+#pragma unroll
+    for (int k = 0; k < QT; ++k) {
+        asm volatile("" : "+d"(g[k]));
+        if (MODE == 2) asm volatile("" : "+d"(h[k]));
     }
     if (MODE == 0) { const double2 d = a.sc[flat0]; c0 = d.x; c1 = d.y; }
     if (MODE == 1) c0 = h[0];
@@ -371,8 +389,8 @@ __global__ void __launch_bounds__(AMP_THREADS, MINB) k_amp(const AmpArgs a)
 }
 
 // lookup functions of the three instantiation units (NULL if the combination is not built)
-amp_kernel_t amp_kernel_direct(int mode, int qt, bool split, int nch, int npoly);
-amp_kernel_t amp_kernel_rec_polar(int qt, int nb, bool split, int nch, bool poly, bool rec3);
-amp_kernel_t amp_kernel_rec_cart(int qt, int nb, bool split, int nch, bool poly, bool rec3);
+amp_kernel_t amp_kernel_direct(int mode, int qt, bool split, int nch, int npoly, bool uni);
+amp_kernel_t amp_kernel_rec_polar(int qt, int nb, bool split, int nch, bool poly, bool rec3, bool uni);
+amp_kernel_t amp_kernel_rec_cart(int qt, int nb, bool split, int nch, bool poly, bool rec3, bool uni);
 
 }  // namespace nms

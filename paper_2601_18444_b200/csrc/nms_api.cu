@@ -548,6 +548,7 @@ nms_status nms_set_option(nms_ctx* c, const char* key, int64_t value)
     else if (!strcmp(key, "chunks")) { if (value < 0) return fail(c, NMS_E_ARG, "chunks must be >= 0"); c->opt_chunks = (int)value; }
     else if (!strcmp(key, "bases")) { if (value < 0 || value > 4) return fail(c, NMS_E_ARG, "bases must be 0..4"); c->opt_bases = (int)value; }
     else if (!strcmp(key, "precision")) { if (value < 0 || value > 2) return fail(c, NMS_E_ARG, "precision must be 0, 1 or 2"); c->opt_precision = (int)value; }
+    else if (!strcmp(key, "uniform")) { c->opt_uniform = (int)value; }
     else if (!strcmp(key, "recurrence")) { if (value < 0 || value > 2) return fail(c, NMS_E_ARG, "recurrence must be 0, 1 or 2"); c->opt_rec3 = (int)value; }
     else if (!strcmp(key, "qt")) { if (value != 0 && value != 4 && value != 8 && value != 16) return fail(c, NMS_E_ARG, "qt must be 0, 4, 8 or 16"); c->opt_qt = (int)value; }
     else return fail(c, NMS_E_ARG, "unknown option '%s'", key);

@@ -63,6 +63,7 @@ struct nms_ctx {
     int opt_qt = 0;        // 0 auto, else 4/8/16
     int opt_bases = 0;     // recurrence kernels: exactly evaluated points per 8 (0 auto = 2, else 1..4)
     int opt_precision = 0; // 0 auto = 1 fast (MUFU phasors), 2 accurate (polynomial phasors)
+    int opt_uniform = 0;   // 1: never use the block-uniform instantiations (testing)
     int opt_rec3 = 0;      // recurrence kernels: 0 auto, 1 rotations, 2 three-term recurrence
     int amp_timer = NMS_T_AMPLITUDE;   // timer class of the amplitude launch (-1: none, the caller times it)
     int64_t launches = 0;
@@ -151,6 +152,7 @@ struct AmpPlan {
     int npoly;         // direct: phasors per thread evaluated by polynomial (qt = all: accurate); recurrence: 0 / 1
     int nb;            // recurrence: exactly evaluated points per thread
     int rec3;          // recurrence: three-term recurrence instead of rotations
+    bool uni;          // n1 % 128 == 0: a block lies inside one group of lines (block-uniform abscissae)
 };
 nms_status plan_amplitude(nms_ctx* c, bool split, AmpPlan* plan);
 nms_status launch_amplitude(nms_ctx* c, const AmpPlan& plan, const int32_t* kinds_dev, int n_kinds);
