@@ -677,6 +677,9 @@ def main():
     ap.add_argument("--shard", default="auto", choices=["auto", "replicas", "lines"],
                     help="N > 1: the detector lines of ONE workload shared by the ranks (strong scaling; DESIGN.md "
                          "section 9) or independent replicas (weak scaling); auto = lines where the workload admits it")
+    ap.add_argument("--pipes", action="store_true",
+                    help="measured issue rates of the instruction classes of the amplitude kernels and error statistics "
+                         "of the two phasor routines (one JSON line; the table behind DESIGN.md section 6)")
     ap.add_argument("--no-configs", action="store_true", help="skip the C3 / C4 side measurements of the default line")
     args = ap.parse_args()
     rank, local_rank, world = _env_int("RANK", 0), _env_int("LOCAL_RANK", 0), _env_int("WORLD_SIZE", 1)
@@ -690,7 +693,19 @@ def main():
             port = sk.getsockname()[1]
         os.execv(sys.executable, [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
                                   "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:])
-    if args.sweep:
+    if args.pipes:
+        if rank == 0:
+            import torch
+            import paper_2601_18444_b200 as nms
+            peaks, src = _peaks()
+            with nms.Context(0) as ctx:
+                rates = nms.nms_pipe_rates(ctx.h)
+                st = {name: nms.nms_phasor_selftest(ctx.h, poly, 24) for name, poly in (("mufu", False), ("polynomial", True))}
+            for v in st.values():
+                v["harmonics"] = {str(k): x for k, x in v["harmonics"].items()}
+            print(json.dumps({"pipes": "operations per clock and SM (16 warps/SM, 8 independent chains, clock64)", "rates": rates,
+                              "phasor_error": st, "gpu": torch.cuda.get_device_name(0), "sm_max_mhz": peaks.get("sm_max_mhz")}), flush=True)
+    elif args.sweep:
         if rank == 0:
             run_sweep(args)
     elif args.impl == "reference":

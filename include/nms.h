@@ -266,6 +266,35 @@ NMS_API nms_status nms_kernel_time_ms(nms_ctx* ctx, nms_timer which, float* ms);
  * This is what bench.py divides the algorithmic work by for the roofline figure.                  */
 NMS_API nms_status nms_kernel_time_total(nms_ctx* ctx, nms_timer which, double* total_ms, int64_t* count);
 
+/* ---- measured properties of the machine and of the phasor routines (diagnostics) ------------------------------------ */
+
+/* Instruction classes timed by nms_pipe_rates, in this order. */
+typedef enum {
+    NMS_PIPE_FFMA = 0,        /* fma.rn.f32                                   lane-FMAs per clock and SM              */
+    NMS_PIPE_FFMA2_REG = 1,   /* fma.rn.f32x2, three 64-bit register operands (2 lane-FMAs per instruction and lane)  */
+    NMS_PIPE_FFMA2_BCAST = 2, /* fma.rn.f32x2 with a broadcast 32-bit operand -- the form the amplitude kernels use   */
+    NMS_PIPE_FMUL = 3,
+    NMS_PIPE_MUFU_SIN = 4,    /* sin.approx (FMUL.RZ + MUFU.SIN)              MUFU per clock and SM                   */
+    NMS_PIPE_MUFU_EX2 = 5,    /* ex2.approx (MUFU.EX2 alone)                                                          */
+    NMS_PIPE_DFMA = 6,
+    NMS_PIPE_I2FP = 7,
+    NMS_PIPE_IALU = 8,        /* SHF + IADD3                                   integer operations per clock and SM    */
+    NMS_PIPE_LOP3 = 9,
+    NMS_PIPE_F2F = 10,        /* double -> float -> double round trip + DMUL   round trips per clock and SM           */
+    NMS_PIPE_PHASOR_MUFU = 11,/* whole MUFU phasor (nms_phasor.cuh)            phasors per clock and SM               */
+    NMS_PIPE_PHASOR_POLY = 12,/* whole polynomial phasor                                                              */
+    NMS_PIPE_COUNT = 13
+} nms_pipe;
+/* Micro-benchmark behind the roofline figures of DESIGN.md section 6: for each class above, 16 warps per SM each run
+ * 8 independent chains of the instruction for 4096 rounds between two clock64() reads; out [host][NMS_PIPE_COUNT]
+ * receives operations per clock and SM (slowest block).  Synchronises.                                                  */
+NMS_API nms_status nms_pipe_rates(nms_ctx* ctx, double* out);
+/* Error statistics of the phasor routine of the amplitude kernels (polynomial = 0: MUFU, 1: polynomial) over 2^log2_n
+ * stratified phases (10 <= log2_n <= 30) against fp64: out [host][21] = largest |error| of cos, of sin, rms error of cos,
+ * of sin, then |e_n| for n = -8 ... 8, the Fourier coefficients of the complex error function e(phi) = z_computed -
+ * exp(-i phi) (e_n multiplies A(n q) in the error of A(q); e_1 is a harmless relative error).  Synchronises.             */
+NMS_API nms_status nms_phasor_selftest(nms_ctx* ctx, int polynomial, int log2_n, double* out);
+
 #ifdef __cplusplus
 }
 #endif

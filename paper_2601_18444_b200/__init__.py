@@ -34,7 +34,7 @@ EXPORTS = [
     "nms_set_rotation", "nms_set_polarization", "nms_set_scales", "nms_amplitudes", "nms_response", "nms_compute",
     "nms_azimuthal_average", "nms_correlation", "nms_form_factor_split", "nms_run_host", "nms_get_weight_sums",
     "nms_set_option", "nms_get_info", "nms_kernel_time_ms", "nms_kernel_time_total", "nms_modal_decomposition",
-    "nms_correlation_2d", "nms_cross_spectra", "nms_run_host_split", "nms_run_host_scan",
+    "nms_correlation_2d", "nms_cross_spectra", "nms_run_host_split", "nms_run_host_scan", "nms_pipe_rates", "nms_phasor_selftest",
 ]
 
 
@@ -253,6 +253,25 @@ def nms_get_weight_sums(ctx) -> np.ndarray:
     out = np.zeros(4, dtype=np.float64)
     _check(ctx, _lib.nms_get_weight_sums(ctx, C.c_void_p(out.ctypes.data)))
     return out
+
+
+PIPES = ["FFMA", "FFMA2_REG", "FFMA2_BCAST", "FMUL", "MUFU_SIN", "MUFU_EX2", "DFMA", "I2FP", "IALU", "LOP3", "F2F",
+         "PHASOR_MUFU", "PHASOR_POLY"]
+
+
+def nms_pipe_rates(ctx) -> dict:
+    """Measured operations per clock and SM of the instruction classes the amplitude kernels are made of."""
+    out = np.zeros(len(PIPES), dtype=np.float64)
+    _check(ctx, _lib.nms_pipe_rates(ctx, C.c_void_p(out.ctypes.data)))
+    return {k: float(v) for k, v in zip(PIPES, out)}
+
+
+def nms_phasor_selftest(ctx, polynomial: bool, log2_n: int = 24) -> dict:
+    """Error statistics of the kernels' phasor routine against fp64 (see include/nms.h)."""
+    out = np.zeros(21, dtype=np.float64)
+    _check(ctx, _lib.nms_phasor_selftest(ctx, C.c_int(1 if polynomial else 0), C.c_int(log2_n), C.c_void_p(out.ctypes.data)))
+    return {"max_cos": out[0], "max_sin": out[1], "rms_cos": out[2], "rms_sin": out[3],
+            "harmonics": {n: float(out[4 + n + 8]) for n in range(-8, 9)}}
 
 
 def nms_set_option(ctx, key: str, value: int):

@@ -265,7 +265,7 @@ void nms_destroy(nms_ctx* c)
     DevBuf* bufs[] = {&c->raw_pos, &c->raw_N, &c->raw_m, &c->centres, &c->tile_src, &c->tile_meta, &c->cells,
                       &c->wsum, &c->u0, &c->u1, &c->qc, &c->sc, &c->amp64, &c->part, &c->formpart,
                       &c->chunk_begin, &c->kinds_dev, &c->bin_idx, &c->bin_sum, &c->bin_cnt, &c->modal_tab, &c->modal_ring,
-                      &c->tile_wsum, &c->pix_cells, &c->pix_meta, &c->pix_u0, &c->pix_u1, &c->pix_qc, &c->pix_sc};
+                      &c->tile_wsum, &c->diag, &c->pix_cells, &c->pix_meta, &c->pix_u0, &c->pix_u1, &c->pix_qc, &c->pix_sc};
     for (DevBuf* b : bufs) free_buf(*b);
     for (DevBuf& b : c->host_stage) free_buf(b);
     if (c->h_geo) cudaFreeHost(c->h_geo);

@@ -115,6 +115,7 @@ struct nms_ctx {
     nms::DevBuf bin_idx, bin_sum, bin_cnt;
     nms::DevBuf pix_cells, pix_meta, pix_u0, pix_u1, pix_qc, pix_sc;   // 2-D correlation: detector pixels as a sample, r-grid
     nms::DevBuf modal_tab, modal_ring; // (sin, cos)(k theta_j) table; fp64 ring values of the modal decomposition
+    nms::DevBuf diag;                  // scratch of the diagnostics (k_diag.cu)
     nms::DevBuf host_stage[8];         // device staging for nms_run_host
 
     nms::Timer timers[NMS_T_COUNT];

@@ -1003,3 +1003,26 @@ def test_run_host_matches_device_path(nms, ctx):
     np.testing.assert_allclose(out_I, I.cpu().numpy(), rtol=1e-6, atol=0)
     np.testing.assert_allclose(out_c, c.cpu().numpy(), rtol=1e-5, atol=1e-7 * np.abs(out_c).max())
     np.testing.assert_allclose(out_p, p.cpu().numpy(), rtol=1e-5, atol=1e-7 * np.abs(out_p).max())
+
+
+def test_phasor_error_statistics(nms, ctx):
+    """The two phasor routines of the amplitude kernels over 2^22 stratified phases against fp64 (nms_phasor_selftest):
+    MUFU within the 2^-21.4 of the CUDA C Programming Guide plus the I2FP / FMUL roundings; the polynomial phasor at
+    fp32 rounding level with every Fourier coefficient of its error function (the leakage of A(n q) into A(q)) below
+    2e-9 -- the figures DESIGN.md section 7 quotes."""
+    mufu = nms.nms_phasor_selftest(ctx, False, 22)
+    poly = nms.nms_phasor_selftest(ctx, True, 22)
+    assert max(mufu["max_cos"], mufu["max_sin"]) <= 6e-7
+    assert max(poly["max_cos"], poly["max_sin"]) <= 1.2e-7
+    assert max(poly["rms_cos"], poly["rms_sin"]) <= 3e-8
+    assert all(v <= 2e-9 for n, v in poly["harmonics"].items())
+    assert mufu["harmonics"][0] <= 2e-8                       # no constant term: nothing of sum w leaks into A(q)
+
+
+def test_pipe_rates_are_sane(nms, ctx):
+    """The micro-benchmark behind the roofline denominators: 128 FP32 lanes and 16 MUFU lanes per clock and SM."""
+    r = nms.nms_pipe_rates(ctx)
+    assert 100.0 <= r["FFMA"] <= 135.0
+    assert 100.0 <= r["FFMA2_BCAST"] <= 130.0              # lane-FMAs: a packed FFMA2 is two of them
+    assert 12.0 <= r["MUFU_EX2"] <= 17.0
+    assert r["PHASOR_POLY"] < r["FFMA"] / 8.0
