@@ -91,6 +91,14 @@ def amplitudes(pos, N, m, R=None, qy=None, qz=None, qx=None, offsets=None, centr
     return (out, wsum) if return_wsum else out
 
 
+def amplitudes_batch(pos, N, m_batch, R=None, qy=None, qz=None, offsets=None, centres=None):
+    """Batched magnetisation fields on a fixed geometry (the paper's loop mode: one m_i file per field / temperature /
+    time step on the same NucData and StructData, L254, L323, L391): the plain loop of `amplitudes` over the B fields
+    m_batch [B, W, 3].  Returns A [B, 8, n_q]; the nuclear planes A[b, 0:2] are the same for every field."""
+    m_batch = np.ascontiguousarray(m_batch, dtype=np.float32)
+    return np.stack([amplitudes(pos, N, m_batch[b], R, qy, qz, offsets=offsets, centres=centres) for b in range(m_batch.shape[0])])
+
+
 def response(amp, theta, kinds: Sequence[int], P=None, sN=1.0, sM=1.0, invV=1.0, return_Q=False):
     """Response maps [n_kinds, n_q] from amplitudes via the Halpern-Johnson vector (Eq. 3-29)."""
     amp, theta = _f64(amp), _f64(theta)

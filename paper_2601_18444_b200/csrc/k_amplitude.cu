@@ -69,6 +69,49 @@ static amp_kernel_t pick_kernel(const AmpPlan& p)
 
 static int64_t ceil_div(int64_t a, int64_t b) { return (a + b - 1) / b; }
 
+// Number of cell chunks.  Measured on B200 (C3, C4, C5): many short blocks beat one long wave (C5 0.759 -> 0.785,
+// C4 0.763 -> 0.813, C3 0.587 -> 0.630 of the roofline from 9 chunks to 16+ waves) -- the blocks are equal-sized, so
+// what counts is that blocks / (SMs x resident blocks) comes out close to a whole number and that there are enough
+// waves for the dynamic scheduler to even out.  Search 16 ... 48 waves for the best product of wave fill and unit
+// balance; the fp64 partials (chunk_bytes per chunk) cap it at 2 GB; at least min_units units of work per chunk.
+int choose_chunks(nms_ctx* c, int64_t n_qb, int64_t slots, int64_t units, double chunk_bytes, int64_t min_units)
+{
+    int64_t max_chunks = units;
+    const int64_t mem_cap = (int64_t)(2.0e9 / chunk_bytes);
+    if (max_chunks > mem_cap) max_chunks = mem_cap < 1 ? 1 : mem_cap;
+    if (max_chunks > 4096) max_chunks = 4096;
+    if (max_chunks > units / min_units) max_chunks = units / min_units < 1 ? 1 : units / min_units;
+    int64_t best_c = 1; double best_eff = -1.0;
+    if (c->opt_chunks > 0) return (int)(c->opt_chunks < units ? c->opt_chunks : units);
+    int64_t lo = ceil_div(16 * slots, n_qb), hi = ceil_div(48 * slots, n_qb);
+    if (lo > max_chunks) lo = 1;                    // small problem: take the best there is
+    if (hi > max_chunks) hi = max_chunks;
+    for (int64_t nc = lo; nc <= hi; ++nc) {
+        const int64_t blocks = n_qb * nc;
+        const double wave_eff = (double)blocks / (double)(ceil_div(blocks, slots) * slots);
+        const double bal_eff = (double)units / (double)(ceil_div(units, nc) * nc);
+        const double eff = wave_eff * bal_eff;
+        if (eff > best_eff + 1e-9) { best_eff = eff; best_c = nc; }
+        if (eff >= 0.995) break;
+    }
+    return (int)best_c;
+}
+
+// Geometry of the packed sample (k_prep) on the host -- waits for the prep pass only -- and the range check of the fp32
+// kernels: the adder-rounding reduction of the phase holds for |t| < 2^19 cycles (nms_phasor.cuh).
+nms_status wait_geometry(nms_ctx* c)
+{
+    if (c->geo_pending) {
+        NMS_CUDA(c, cudaEventSynchronize(c->geo_event));
+        c->geo_rmax = c->h_geo[0]; c->geo_ext = c->h_geo[1]; c->geo_extz = c->h_geo[2];
+        c->geo_pending = false;
+    }
+    if (c->g_qmax * c->geo_rmax * INV_2PI >= 524288.0 * 0.99)
+        return fail(c, NMS_E_UNSUPPORTED, "q_max r_max / 2 pi = %.3g cycles exceeds 2^19: use the exact kernel (variant 3)",
+                    c->g_qmax * c->geo_rmax * INV_2PI);
+    return NMS_OK;
+}
+
 nms_status plan_amplitude(nms_ctx* c, bool split, AmpPlan* plan)
 {
     // precision policy: small problems run the exact fp64 kernel; otherwise the line
@@ -86,16 +129,7 @@ nms_status plan_amplitude(nms_ctx* c, bool split, AmpPlan* plan)
     else if (c->opt_variant == 2 || (c->opt_variant == 0 && line_ok)) p.variant = (c->g_type == 0) ? 3 : 5;
     else p.variant = (c->g_type == 0) ? 2 : 4;
     if (p.variant != 8) {
-        // geometry of the packed sample (k_prep): waits for the prep pass only
-        if (c->geo_pending) {
-            NMS_CUDA(c, cudaEventSynchronize(c->geo_event));
-            c->geo_rmax = c->h_geo[0]; c->geo_ext = c->h_geo[1]; c->geo_extz = c->h_geo[2];
-            c->geo_pending = false;
-        }
-        // the adder-rounding reduction of the phase holds for |t| < 2^19 cycles (nms_phasor.cuh)
-        if (c->g_qmax * c->geo_rmax * INV_2PI >= 524288.0 * 0.99)
-            return fail(c, NMS_E_UNSUPPORTED, "q_max r_max / 2 pi = %.3g cycles exceeds 2^19: use the exact kernel (variant 3)",
-                        c->g_qmax * c->geo_rmax * INV_2PI);
+        if (nms_status st = wait_geometry(c)) return st;
         // automatic choice: after its first-order correction at the tile centres the recurrence leaves a phase error
         // <= (deviation of the float abscissae from the progression) x (half extent of a tile along the line's
         // direction: any direction of the detector plane for a polar grid, Z for a Cartesian one); beyond 2e-5 rad
@@ -151,34 +185,8 @@ nms_status plan_amplitude(nms_ctx* c, bool split, AmpPlan* plan)
     const int64_t n_qb = p.variant == 8 ? ceil_div(c->n_q, AMP_THREADS)
                                         : ceil_div(ceil_div(c->g_n0, p.qt) * c->g_n1, AMP_THREADS);
 
-    // number of cell chunks.  Measured on B200 (C3, C4, C5): many short blocks beat one long wave (C5 0.759 -> 0.785,
-    // C4 0.763 -> 0.813, C3 0.587 -> 0.630 of the roofline from 9 chunks to 16+ waves) -- the blocks are equal-sized, so
-    // what counts is that blocks / (SMs x resident blocks) comes out close to a whole number and that there are enough
-    // waves for the dynamic scheduler to even out.  Search 16 ... 48 waves for the best product of wave fill and unit
-    // balance; the fp64 partials (64 B, in split mode (8 + n_kinds) * 8 B, per detector point and chunk) cap it at 2 GB.
-    int64_t max_chunks = units;
-    const double chunk_bytes = 8.0 * (double)c->n_q * (split ? 8.0 + NMS_KIND_COUNT : 8.0);
-    const int64_t mem_cap = (int64_t)(2.0e9 / chunk_bytes);
-    if (max_chunks > mem_cap) max_chunks = mem_cap < 1 ? 1 : mem_cap;
-    if (max_chunks > 4096) max_chunks = 4096;
-    const int64_t min_units = split ? 1 : 8;            // at least 8 tiles per block
-    if (max_chunks > units / min_units) max_chunks = units / min_units < 1 ? 1 : units / min_units;
-    int64_t best_c = 1; double best_eff = -1.0;
-    if (c->opt_chunks > 0) best_c = c->opt_chunks < units ? c->opt_chunks : units;
-    else {
-        int64_t lo = ceil_div(16 * slots, n_qb), hi = ceil_div(48 * slots, n_qb);
-        if (lo > max_chunks) lo = 1;                    // small problem: take the best there is
-        if (hi > max_chunks) hi = max_chunks;
-        for (int64_t nc = lo; nc <= hi; ++nc) {
-            const int64_t blocks = n_qb * nc;
-            const double wave_eff = (double)blocks / (double)(ceil_div(blocks, slots) * slots);
-            const double bal_eff = (double)units / (double)(ceil_div(units, nc) * nc);
-            const double eff = wave_eff * bal_eff;
-            if (eff > best_eff + 1e-9) { best_eff = eff; best_c = nc; }
-            if (eff >= 0.995) break;
-        }
-    }
-    p.n_chunks = (int)best_c; p.n_qblocks = (int)n_qb; p.blocks_per_sm = occ;
+    p.n_chunks = choose_chunks(c, n_qb, slots, units, 8.0 * (double)c->n_q * (split ? 8.0 + NMS_KIND_COUNT : 8.0), split ? 1 : 8);
+    p.n_qblocks = (int)n_qb; p.blocks_per_sm = occ;
     *plan = p;
     return NMS_OK;
 }

@@ -156,6 +156,8 @@ struct AmpPlan {
     bool uni;          // n1 % 128 == 0: a block lies inside one group of lines (block-uniform abscissae)
 };
 nms_status plan_amplitude(nms_ctx* c, bool split, AmpPlan* plan);
+int choose_chunks(nms_ctx* c, int64_t n_qb, int64_t slots, int64_t units, double chunk_bytes, int64_t min_units);
+nms_status wait_geometry(nms_ctx* c);                     // r_max / tile extents of the packed sample (k_prep) on the host
 nms_status launch_amplitude(nms_ctx* c, const AmpPlan& plan, const int32_t* kinds_dev, int n_kinds);
 // k_epilogue.cu
 nms_status launch_epilogue(nms_ctx* c, int n_chunks, const int32_t* kinds_dev, int n_kinds, float* out_maps,

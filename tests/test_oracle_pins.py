@@ -760,3 +760,37 @@ def test_cross_spectra_uniform_magnetisation(oracle_mod):
         for b in range(3):
             np.testing.assert_allclose(GR[3 * a + b], n[a] * n[b] * F2, rtol=1e-6, atol=1e-9 * F2.max())
             assert np.abs(GI[3 * a + b]).max() <= 1e-9 * F2.max()
+
+
+# --------------------------------------------------------------------------- f-3: batched magnetisation fields
+def test_batched_fields_share_the_nuclear_amplitude_and_are_linear(oracle_mod):
+    """Loop mode (L254, L323, L391): B magnetisation fields on one geometry.  Pins that do not re-call the routine on the
+    same data: (i) the nuclear planes do not depend on the field and equal the run without moments; (ii) M~ is linear in
+    m -- fields chosen with exactly representable sums, m_2 = m_0 + m_1 and m_3 = -2 m_0; (iii) a uniform field m_b = n_b
+    on N = 1 has M~ = (R n_b) N~ (Eq. 43 with constant moment); (iv) B = 1 is the single call."""
+    rng = np.random.Generator(np.random.Philox(33))
+    W = 257
+    pos = rng.uniform(-12, 12, size=(W, 3)).astype(np.float32)
+    N = np.ones(W, dtype=np.float32)
+    m0 = (rng.integers(-8, 9, size=(W, 3)) / 8.0).astype(np.float32)            # dyadic: sums are exact in fp32
+    m1 = (rng.integers(-8, 9, size=(W, 3)) / 16.0).astype(np.float32)
+    n4, n5 = np.array([0.25, -0.5, 1.0], dtype=np.float32), np.array([1.0, 0.0, 0.0], dtype=np.float32)
+    mb = np.stack([m0, m1, m0 + m1, -2.0 * m0, np.tile(n4, (W, 1)), np.tile(n5, (W, 1))]).astype(np.float32)
+    R = ni.rotation_alpha_beta(25.0, 40.0)
+    g = _polar(7, 9)
+    qy, qz, th = oracle_mod.grid_points(g)
+    A = oracle_mod.amplitudes_batch(pos, N, mb, R, qy, qz)
+    assert A.shape == (6, 8, g.n_q)
+    A_nuc = oracle_mod.amplitudes(pos, N, None, R, qy, qz)
+    scale = np.abs(A).max()
+    for b in range(6):
+        np.testing.assert_allclose(A[b, 0:2], A_nuc[0:2], rtol=0, atol=1e-13 * scale)                 # (i)
+    np.testing.assert_allclose(A[2, 2:], A[0, 2:] + A[1, 2:], rtol=0, atol=1e-12 * scale)             # (ii)
+    np.testing.assert_allclose(A[3, 2:], -2.0 * A[0, 2:], rtol=0, atol=1e-12 * scale)
+    for b, n in ((4, n4), (5, n5)):                                                                   # (iii)
+        Rn = R @ n.astype(np.float64)
+        for c in range(3):
+            np.testing.assert_allclose(A[b, 2 + 2 * c], Rn[c] * A_nuc[0], rtol=0, atol=1e-12 * scale)
+            np.testing.assert_allclose(A[b, 3 + 2 * c], Rn[c] * A_nuc[1], rtol=0, atol=1e-12 * scale)
+    A1 = oracle_mod.amplitudes_batch(pos, N, mb[1:2], R, qy, qz)                                      # (iv)
+    assert np.array_equal(A1[0], oracle_mod.amplitudes(pos, N, mb[1], R, qy, qz))
