@@ -249,7 +249,7 @@ class Runner:
         self.ctx.close()
 
 
-def time_next_rows(nms, run, wl, torch, dev, reps=3):
+def time_next_rows(nms, run, wl, torch, dev, reps=3, step_ms=None):
     """SURVEY 8(f) rows built so far, timed OUTSIDE the step on the step's last maps (polar detectors only):
     f-2 angular modal decomposition of all maps (k_max = 8) and f-1 two-dimensional correlation function of the
     first map on a (rho, alpha) grid of the detector's own size -- the amplitude kernel with pixels as cells."""
@@ -269,6 +269,20 @@ def time_next_rows(nms, run, wl, torch, dev, reps=3):
         fn()
         ms = _timed(torch, dev, fn, reps) / reps
         out[name] = {"ms": ms, "units": units, "gunits_per_s": units / (ms * 1e-3) / 1e9}
+    # f-3: B = 6 magnetisation fields (two passes of 3) on the workload's geometry; the fields are the sample's own
+    # moments with permuted components and flipped signs (made on the device; the kernel cannot tell)
+    if run.d_m is not None:
+        B = 6
+        mb = torch.stack([torch.roll(run.d_m, b % 3, dims=1) * (1.0 if b < 3 else -1.0) for b in range(B)]).contiguous()
+        bmaps = torch.empty((B, nk, g.n_q), **f32)
+        fn = lambda: nms.nms_compute_batch(h, wl.grid, mb, wl.kinds, bmaps, None)
+        fn()
+        ms = _timed(torch, dev, fn, 1)
+        units = B * wl.W * g.n_q
+        out["batched_fields_f3"] = {"ms": ms, "fields": B, "units": units, "gunits_per_s": units / (ms * 1e-3) / 1e9,
+                                    "unit": "cell x q x field triples (shared phasor and nuclear sum; whole call incl. packing and responses)",
+                                    "speedup_vs_single_field_step": (units / ms) / (wl.pairs / wl.n_rot / step_ms) if step_ms else None}
+        del mb, bmaps
     out["modal_f2"]["unit"] = "map values x harmonics"
     out["correlation_2d_f1"]["unit"] = "pixel x r-point pairs (one complex amplitude)"
     out["correlation_2d_f1"]["r_grid"] = f"polar {rgrid.n0}x{rgrid.n1}, rho <= {r_max:.1f}"
@@ -596,7 +610,7 @@ def measure(nms, torch, wl_full, args, steps, warmup, dist, rank, local_rank, wo
         h2d, d2h = run.bytes_per_step()
         res["e2e"] = {"value": aggregate_rate(wl_full.pairs, 1 if sharded else world, ms_e2e), "unit": "Gpair/s",
                       "ms_per_step": ms_e2e, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": e2e_steps}
-        res["next_rows"] = time_next_rows(nms, run, wl, torch, dev) if (wl.grid.type == 0 and not sharded) else None
+        res["next_rows"] = time_next_rows(nms, run, wl, torch, dev, step_ms=ms_step) if (wl.grid.type == 0 and not sharded) else None
     # the maps of the FIRST rotation of one more (untimed) pass, for the parity object
     maps_host = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:

@@ -94,7 +94,8 @@ typedef enum {
     NMS_T_CORRELATION = 4,  /* a-5                                                  */
     NMS_T_MODAL = 5,        /* f-2 angular modal decomposition                      */
     NMS_T_CORR2D = 6,       /* f-1 two-dimensional correlation function (its amplitude kernel) */
-    NMS_T_COUNT = 7
+    NMS_T_BATCH = 7,        /* f-3 amplitude kernel of the batched magnetisation fields */
+    NMS_T_COUNT = 8
 } nms_timer;
 
 /* ---- context ---------------------------------------------------------------------------------- */
@@ -150,6 +151,17 @@ NMS_API nms_status nms_cross_spectra(nms_ctx* ctx, float* out_GR, float* out_GI)
 /* Fused a-2 + a-3: amplitudes and all requested responses without materialising the amplitudes.
  * This is the call bench.py times.  out [dev][n_kinds][n_q] (float).                             */
 NMS_API nms_status nms_compute(nms_ctx* ctx, const nms_qgrid* grid, const nms_kind* kinds, int n_kinds, float* out);
+
+/* ---- batched magnetisation fields on a fixed geometry (f-3; the paper's loop mode L254, L323, L391, L686) -------- */
+
+/* n_fields magnetisation fields m_batch [dev][n_fields][W][3] on the geometry of the current sample (positions, N, object
+ * centres and rotation as set by nms_set_sample / nms_set_particles / nms_set_rotation; the sample's own m is not used).
+ * The phasors and the nuclear sum are evaluated once per group of 3 fields and shared; field b gets the same results as
+ * nms_set_sample(pos, N, m_batch[b]) + nms_compute would give.  out_maps [dev][n_fields][n_kinds][n_q] (float) or NULL;
+ * out_amp [dev][n_fields][8][n_q] (float, plane order as nms_amplitudes; planes 0-1 are the shared nuclear amplitude) or
+ * NULL (not both NULL).  fp32 kernels with MUFU phasors (as the direct kernel of nms_compute) at every problem size.  */
+NMS_API nms_status nms_compute_batch(nms_ctx* ctx, const nms_qgrid* grid, const float* m_batch, int n_fields,
+                             const nms_kind* kinds, int n_kinds, float* out_maps, float* out_amp);
 
 /* ---- azimuthal average (a-4, Eq. 30) ------------------------------------------------------ */
 

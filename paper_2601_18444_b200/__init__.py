@@ -26,7 +26,7 @@ LIB_PATH = os.path.join(_HERE, "libnms.so")
 
 KINDS = ["NUC", "MAG", "UNPOL", "PROJ", "NM", "SF", "CHI", "PM", "MP", "PP", "MM", "POL_PLUS", "POL_MINUS"]
 NMS_OK, NMS_E_ARG, NMS_E_STATE, NMS_E_CUDA, NMS_E_NOMEM, NMS_E_UNSUPPORTED = range(6)
-NMS_T_PREP, NMS_T_AMPLITUDE, NMS_T_EPILOGUE, NMS_T_AZIMUTHAL, NMS_T_CORRELATION, NMS_T_MODAL, NMS_T_CORR2D = range(7)
+NMS_T_PREP, NMS_T_AMPLITUDE, NMS_T_EPILOGUE, NMS_T_AZIMUTHAL, NMS_T_CORRELATION, NMS_T_MODAL, NMS_T_CORR2D, NMS_T_BATCH = range(8)
 _STATUS = {0: "NMS_OK", 1: "NMS_E_ARG", 2: "NMS_E_STATE", 3: "NMS_E_CUDA", 4: "NMS_E_NOMEM", 5: "NMS_E_UNSUPPORTED"}
 
 EXPORTS = [
@@ -34,7 +34,7 @@ EXPORTS = [
     "nms_set_rotation", "nms_set_polarization", "nms_set_scales", "nms_amplitudes", "nms_response", "nms_compute",
     "nms_azimuthal_average", "nms_correlation", "nms_form_factor_split", "nms_run_host", "nms_get_weight_sums",
     "nms_set_option", "nms_get_info", "nms_kernel_time_ms", "nms_kernel_time_total", "nms_modal_decomposition",
-    "nms_correlation_2d", "nms_cross_spectra", "nms_run_host_split", "nms_run_host_scan", "nms_pipe_rates", "nms_phasor_selftest",
+    "nms_correlation_2d", "nms_cross_spectra", "nms_run_host_split", "nms_run_host_scan", "nms_pipe_rates", "nms_phasor_selftest", "nms_compute_batch",
 ]
 
 
@@ -174,6 +174,14 @@ def nms_compute(ctx, grid, kinds, out):
     g, keep = _grid_struct(grid)
     k, n = _kinds(kinds)
     _check(ctx, _lib.nms_compute(ctx, C.byref(g), k, C.c_int(n), _dev(out)))
+
+
+def nms_compute_batch(ctx, grid, m_batch, kinds, out_maps=None, out_amp=None):
+    """Batched magnetisation fields m_batch [B, W, 3] (CUDA tensor) on the current sample's geometry (f-3)."""
+    g, keep = _grid_struct(grid)
+    k, n = _kinds(kinds)
+    _check(ctx, _lib.nms_compute_batch(ctx, C.byref(g), _dev(m_batch), C.c_int(int(m_batch.shape[0])), k, C.c_int(n),
+                                       _dev(out_maps), _dev(out_amp)))
 
 
 def nms_form_factor_split(ctx, grid, kinds, out_total, out_form):

@@ -265,7 +265,7 @@ void nms_destroy(nms_ctx* c)
     DevBuf* bufs[] = {&c->raw_pos, &c->raw_N, &c->raw_m, &c->centres, &c->tile_src, &c->tile_meta, &c->cells,
                       &c->wsum, &c->u0, &c->u1, &c->qc, &c->sc, &c->amp64, &c->part, &c->formpart,
                       &c->chunk_begin, &c->kinds_dev, &c->bin_idx, &c->bin_sum, &c->bin_cnt, &c->modal_tab, &c->modal_ring,
-                      &c->tile_wsum, &c->diag, &c->pix_cells, &c->pix_meta, &c->pix_u0, &c->pix_u1, &c->pix_qc, &c->pix_sc};
+                      &c->tile_wsum, &c->diag, &c->batch_cells, &c->batch_ampN, &c->pix_cells, &c->pix_meta, &c->pix_u0, &c->pix_u1, &c->pix_qc, &c->pix_sc};
     for (DevBuf* b : bufs) free_buf(*b);
     for (DevBuf& b : c->host_stage) free_buf(b);
     if (c->h_geo) cudaFreeHost(c->h_geo);
@@ -393,6 +393,21 @@ nms_status nms_compute(nms_ctx* c, const nms_qgrid* grid, const nms_kind* kinds,
     c->amp_valid = false;
     if (nms_status st = amplitudes_common(c, grid, false, kd, n_kinds, &n_chunks)) return st;
     return launch_epilogue(c, n_chunks, kd, n_kinds, out, nullptr, false);
+}
+
+nms_status nms_compute_batch(nms_ctx* c, const nms_qgrid* grid, const float* m_batch, int n_fields, const nms_kind* kinds,
+                             int n_kinds, float* out_maps, float* out_amp)
+{
+    CHECK_CTX(c);
+    if (!c->packed_valid) return fail(c, NMS_E_STATE, "no sample: call nms_set_sample first (its positions, N, particles and rotation are the fixed geometry)");
+    if (!m_batch || n_fields <= 0) return fail(c, NMS_E_ARG, "m_batch NULL or n_fields <= 0");
+    if (!out_maps && !out_amp) return fail(c, NMS_E_ARG, "no output requested");
+    if (out_maps && n_kinds <= 0) return fail(c, NMS_E_ARG, "out_maps needs n_kinds > 0");
+    const int32_t* kd = nullptr;
+    if (nms_status st = upload_kinds(c, kinds, out_maps ? n_kinds : 0, &kd)) return st;
+    if (nms_status st = set_grid(c, grid)) return st;
+    c->amp_valid = false;
+    return launch_batch(c, m_batch, n_fields, kd, n_kinds, out_maps, out_amp);
 }
 
 nms_status nms_form_factor_split(nms_ctx* c, const nms_qgrid* grid, const nms_kind* kinds, int n_kinds, float* out_total,

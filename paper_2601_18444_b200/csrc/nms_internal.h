@@ -115,6 +115,7 @@ struct nms_ctx {
     nms::DevBuf bin_idx, bin_sum, bin_cnt;
     nms::DevBuf pix_cells, pix_meta, pix_u0, pix_u1, pix_qc, pix_sc;   // 2-D correlation: detector pixels as a sample, r-grid
     nms::DevBuf modal_tab, modal_ring; // (sin, cos)(k theta_j) table; fp64 ring values of the modal decomposition
+    nms::DevBuf batch_cells, batch_ampN;   // f-3: packed records of one pass of fields; the shared nuclear amplitude (fp64)
     nms::DevBuf diag;                  // scratch of the diagnostics (k_diag.cu)
     nms::DevBuf host_stage[8];         // device staging for nms_run_host
 
@@ -166,6 +167,9 @@ nms_status launch_cross_spectra(nms_ctx* c, float* out_GR, float* out_GI);
 nms_status launch_response_from_amp(nms_ctx* c, const int32_t* kinds_dev, int n_kinds, float* out_maps);
 nms_status launch_split_epilogue(nms_ctx* c, int n_chunks, const int32_t* kinds_dev, int n_kinds, float* out_total,
                                  float* out_form);
+// k_batch.cu
+nms_status launch_batch(nms_ctx* c, const float* m_batch, int B, const int32_t* kinds_dev, int n_kinds, float* out_maps,
+                        float* out_amp);
 // k_post.cu
 nms_status launch_azimuthal(nms_ctx* c, const float* maps, int n_maps, int n_bins, double q_lo, double q_hi,
                             float* out_I, float* out_q, int32_t* out_count);

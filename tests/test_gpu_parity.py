@@ -1026,3 +1026,64 @@ def test_pipe_rates_are_sane(nms, ctx):
     assert 100.0 <= r["FFMA2_BCAST"] <= 130.0              # lane-FMAs: a packed FFMA2 is two of them
     assert 12.0 <= r["MUFU_EX2"] <= 17.0
     assert r["PHASOR_POLY"] < r["FFMA"] / 8.0
+
+
+@pytest.mark.parametrize("gtype", [0, 1, 2])
+def test_batched_fields(nms, ctx, oracle_mod, gtype):
+    """f-3 (L254, L323, L391): B = 5 magnetisation fields (two passes: 3 + 2) on the geometry of the reduced C5, with a
+    rotation: amplitudes of every field within 1e-5 sum|w| and all 13 kinds at the north_star criterion against the plain
+    loop of the oracle; the nuclear planes are shared.  Polar, Cartesian and list detectors."""
+    import torch
+    wl = ni.make_config("C5", small=True)
+    rng = np.random.Generator(np.random.Philox(808))
+    B, W = 5, wl.W
+    mb = np.stack([wl.m, np.roll(wl.m, 1, axis=1), -wl.m[:, ::-1], rng.normal(size=(W, 3)),
+                   np.tile(np.array([0.0, 0.6, 0.8]), (W, 1))]).astype(np.float32)
+    R = ni.rotation_alpha_beta(15.0, 35.0)
+    grid = [wl.grid, ni.cartesian_grid(np.linspace(-1.4, 1.5, 19), np.linspace(-1.5, 1.5, 40)),
+            ni.list_grid(rng.uniform(-2, 2, size=301), rng.uniform(-2, 2, size=301))][gtype]
+    kinds = list(ni.ALL_KINDS)
+    nms.nms_set_sample(ctx, _t(wl.pos), _t(wl.N), None, R)
+    nq = grid.n_q
+    maps = torch.empty((B, len(kinds), nq), dtype=torch.float32, device="cuda")
+    amp = torch.empty((B, 8, nq), dtype=torch.float32, device="cuda")
+    nms.nms_compute_batch(ctx, grid, _t(mb), kinds, maps, amp)
+    nms.nms_synchronize(ctx)
+    qy, qz, th = oracle_mod.grid_points(grid)
+    A = oracle_mod.amplitudes_batch(wl.pos, wl.N, mb, R, qy, qz)
+    a_h, m_h = amp.cpu().numpy(), maps.cpu().numpy()
+    misses = []
+    for b in range(B):
+        _, wsum = oracle_mod.amplitudes(wl.pos, wl.N, mb[b], R, qy[:1], qz[:1], return_wsum=True)
+        assert_amplitudes(a_h[b], A[b], wsum, f"field {b}")
+        assert np.array_equal(a_h[b, 0:2], a_h[0, 0:2])                              # one nuclear amplitude for all fields
+        M = oracle_mod.response(A[b], th, kinds)
+        assert_cross_sections(m_h[b], M, kinds, f"field {b}", signed_misses=misses)
+    # the ordinary path on field 3 gives the same maps within the criterion
+    nms.nms_set_sample(ctx, _t(wl.pos), _t(wl.N), _t(mb[3]), R)
+    nms.nms_set_option(ctx, "variant", 1)
+    one = torch.empty((len(kinds), nq), dtype=torch.float32, device="cuda")
+    nms.nms_compute(ctx, grid, kinds, one)
+    nms.nms_synchronize(ctx)
+    pos_k = [i for i, k in enumerate(kinds) if k not in SIGNED]
+    np.testing.assert_allclose(one.cpu().numpy()[pos_k], m_h[3][pos_k], rtol=2e-3, atol=1e-6 * np.abs(m_h[3]).max())
+    report_signed_misses(misses)
+
+
+def test_batched_fields_errors(nms, ctx):
+    import torch
+    wl = ni.make_config("C1")
+    out = torch.empty((1, 1, wl.grid.n_q), dtype=torch.float32, device="cuda")
+    mb = _t(wl.m[None])
+    with pytest.raises(nms.NmsError) as e:
+        nms.nms_compute_batch(ctx, wl.grid, mb, [0], out, None)
+    assert e.value.status == nms.NMS_E_STATE                       # no sample (geometry) yet
+    nms.nms_set_sample(ctx, _t(wl.pos), _t(wl.N), None, None)
+    with pytest.raises(nms.NmsError) as e:
+        nms.nms_compute_batch(ctx, wl.grid, mb, [0], None, None)
+    assert e.value.status == nms.NMS_E_ARG
+    with pytest.raises(nms.NmsError) as e:
+        nms.nms_compute_batch(ctx, wl.grid, mb, [77], out, None)
+    assert e.value.status == nms.NMS_E_ARG
+    nms.nms_compute_batch(ctx, wl.grid, mb, [0], out, None)
+    nms.nms_synchronize(ctx)
