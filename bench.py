@@ -283,6 +283,17 @@ def time_next_rows(nms, run, wl, torch, dev, reps=3, step_ms=None):
                                     "unit": "cell x q x field triples (shared phasor and nuclear sum; whole call incl. packing and responses)",
                                     "speedup_vs_single_field_step": (units / ms) / (wl.pairs / wl.n_rot / step_ms) if step_ms else None}
         del mb, bmaps
+    # f-4: Friedel halving, an EFFECTIVE rate (half of the pairs are taken from A(-q) = A(q)^*); never the headline
+    nms.nms_set_option(h, "friedel", 1)
+    try:
+        fn = lambda: nms.nms_compute(h, wl.grid, wl.kinds, run.maps)
+        fn()
+        ms = _timed(torch, dev, fn, 2) / 2
+        out["friedel_f4"] = {"ms": ms, "effective_gpair_s": wl.W * g.n_q / (ms * 1e-3) / 1e9, "evaluated_gpair_s": 0.5 * wl.W * g.n_q / (ms * 1e-3) / 1e9,
+                             "unit": "EFFECTIVE cell x q pairs per second of nms_compute with option friedel = 1 (half evaluated, half by conjugation)"}
+    except nms.NmsError as e:
+        out["friedel_f4"] = {"unavailable": str(e)}
+    nms.nms_set_option(h, "friedel", 0)
     out["modal_f2"]["unit"] = "map values x harmonics"
     out["correlation_2d_f1"]["unit"] = "pixel x r-point pairs (one complex amplitude)"
     out["correlation_2d_f1"]["r_grid"] = f"polar {rgrid.n0}x{rgrid.n1}, rho <= {r_max:.1f}"

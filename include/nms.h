@@ -262,7 +262,12 @@ NMS_API nms_status nms_get_weight_sums(nms_ctx* ctx, double* out);
  * 1..4).  "recurrence": 0 auto, 1 complex rotations, 2 three-term recurrence (bases <= 2).  "timing": 1 records a
  * CUDA event pair around every kernel launch (and resets the record).  "chunks": 0 auto, else the number of cell
  * chunks.  "qt": 0 auto, else detector points per thread (4 or 8; 16 for the recurrence kernel on a sample without
- * moments).  Unknown keys: NMS_E_ARG.  The fp32 kernels need q_max r_max / 2 pi < 2^19 cycles (NMS_E_UNSUPPORTED
+ * moments).  "friedel" (f-4): 1 = on a polar grid with an even number of angles closed under theta -> theta + pi
+ * (within one ulp of 2 pi; NMS_E_UNSUPPORTED otherwise, and for nms_form_factor_split) the amplitude sums are evaluated
+ * for the first half of every ring only and the second half is taken as the conjugate, A(-q) = A(q)^* for real weights
+ * (Eq. 42-43): half the pair evaluations; the second half then belongs to the float angle rotated by
+ * its deviation from theta + pi (<= 2.4e-7 rad).  Off by default; bench.py reports it as an EFFECTIVE rate only.
+ * Unknown keys: NMS_E_ARG.  The fp32 kernels need q_max r_max / 2 pi < 2^19 cycles (NMS_E_UNSUPPORTED
  * otherwise; the exact kernel has no such limit).                                                        */
 NMS_API nms_status nms_set_option(nms_ctx* ctx, const char* key, int64_t value);
 /* Read back integers: "launches" (kernels launched by this context so far), "variant_used" (1 list direct,

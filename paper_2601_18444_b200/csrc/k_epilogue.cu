@@ -13,6 +13,8 @@ struct EpiArgs {
     const int32_t* kinds;
     int n_kinds, n_chunks;
     int64_t n_q;
+    int64_t n_q_part;       // detector points of the partials (= n_q, or n_q / 2 under Friedel halving)
+    int friedel_n1;         // 0, or n1 of the polar grid whose second half of every ring is the conjugate of the first
     float* out_maps;        // [n_kinds][n_q] or NULL
     float* out_form;        // split: [n_kinds][n_q] or NULL
     float* out_amp;         // [8][n_q] or NULL
@@ -28,9 +30,18 @@ __global__ void __launch_bounds__(256) k_epilogue(const EpiArgs a)
 #pragma unroll
     for (int r = 0; r < 8; ++r) A[r] = 0.0;
     if (a.part) {
+        // Friedel halving (f-4): real weights give A(-q) = A(q)^* (Eq. 42-43), and on a ring theta -> theta + pi is -q
+        int64_t fs = f;
+        bool conj = false;
+        if (a.friedel_n1) {
+            const int64_t i = f / a.friedel_n1, j = f % a.friedel_n1, hn = a.friedel_n1 / 2;
+            conj = j >= hn;
+            fs = i * hn + (conj ? j - hn : j);
+        }
         for (int ch = 0; ch < a.n_chunks; ++ch)
 #pragma unroll
-            for (int r = 0; r < 8; ++r) A[r] += a.part[((int64_t)ch * 8 + r) * a.n_q + f];
+            for (int r = 0; r < 8; ++r) A[r] += a.part[((int64_t)ch * 8 + r) * a.n_q_part + fs];
+        if (conj) { A[1] = -A[1]; A[3] = -A[3]; A[5] = -A[5]; A[7] = -A[7]; }
     } else {
 #pragma unroll
         for (int r = 0; r < 8; ++r) A[r] = a.amp64[(int64_t)r * a.n_q + f];
@@ -116,6 +127,7 @@ nms_status launch_epilogue(nms_ctx* c, int n_chunks, const int32_t* kinds_dev, i
     EpiArgs a = {};
     a.part = (const double*)c->part.p; a.sc = (const double2*)c->sc.p; a.kinds = kinds_dev;
     a.n_kinds = n_kinds; a.n_chunks = n_chunks; a.n_q = c->n_q;
+    a.n_q_part = c->friedel_active ? c->n_q / 2 : c->n_q; a.friedel_n1 = c->friedel_active ? c->g_n1 : 0;
     a.out_maps = out_maps; a.out_amp = out_amp;
     if (keep_amp64) {
         if (nms_status st = ensure(c, c->amp64, sizeof(double) * 8 * (size_t)c->n_q)) return st;
@@ -139,7 +151,7 @@ nms_status launch_split_epilogue(nms_ctx* c, int n_chunks, const int32_t* kinds_
 {
     EpiArgs a = {};
     a.part = (const double*)c->part.p; a.formpart = (const double*)c->formpart.p; a.sc = (const double2*)c->sc.p;
-    a.kinds = kinds_dev; a.n_kinds = n_kinds; a.n_chunks = n_chunks; a.n_q = c->n_q;
+    a.kinds = kinds_dev; a.n_kinds = n_kinds; a.n_chunks = n_chunks; a.n_q = c->n_q; a.n_q_part = c->n_q;
     a.out_maps = out_total; a.out_form = out_form;
     fill_rp(c, a.rp);
     return run(c, a);

@@ -265,7 +265,7 @@ void nms_destroy(nms_ctx* c)
     DevBuf* bufs[] = {&c->raw_pos, &c->raw_N, &c->raw_m, &c->centres, &c->tile_src, &c->tile_meta, &c->cells,
                       &c->wsum, &c->u0, &c->u1, &c->qc, &c->sc, &c->amp64, &c->part, &c->formpart,
                       &c->chunk_begin, &c->kinds_dev, &c->bin_idx, &c->bin_sum, &c->bin_cnt, &c->modal_tab, &c->modal_ring,
-                      &c->tile_wsum, &c->diag, &c->batch_cells, &c->batch_ampN, &c->pix_cells, &c->pix_meta, &c->pix_u0, &c->pix_u1, &c->pix_qc, &c->pix_sc};
+                      &c->tile_wsum, &c->qc_half, &c->sc_half, &c->diag, &c->batch_cells, &c->batch_ampN, &c->pix_cells, &c->pix_meta, &c->pix_u0, &c->pix_u1, &c->pix_qc, &c->pix_sc};
     for (DevBuf* b : bufs) free_buf(*b);
     for (DevBuf& b : c->host_stage) free_buf(b);
     if (c->h_geo) cudaFreeHost(c->h_geo);
@@ -342,14 +342,63 @@ nms_status nms_set_scales(nms_ctx* c, double sN, double sM, double invV)
     return NMS_OK;
 }
 
+// Friedel halving (f-4; Eq. 42-43 L353-L356 with real weights: A(-q) = A(q)^*; L183: the theta grid closes under
+// theta -> theta + pi): the rings' second halves are the point reflections of the first.  Admitted on a polar grid with an
+// even number of angles whose float values satisfy theta[j + n1/2] = theta[j] + pi within one ulp of 2 pi; the second half
+// then carries the direction of its float angle rotated by that deviation (<= 2.4e-7 rad).
+static bool friedel_admissible(const nms_ctx* c)
+{
+    if (c->g_type != 0 || c->g_n1 < 2 || (c->g_n1 & 1)) return false;
+    const int hn = c->g_n1 / 2;
+    for (int j = 0; j < hn; ++j)
+        if (fabs((double)c->h_u1[j + hn] - (double)c->h_u1[j] - 3.14159265358979323846) > 4.8e-7) return false;
+    return true;
+}
+
+__global__ void k_half_rings(const double2* __restrict__ qc, const double2* __restrict__ sc, int n0, int n1,
+                             double2* __restrict__ qc_h, double2* __restrict__ sc_h)
+{
+    const int hn = n1 / 2;
+    const int64_t f = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (f >= (int64_t)n0 * hn) return;
+    const int64_t src = (f / hn) * n1 + (f % hn);
+    qc_h[f] = qc[src];
+    sc_h[f] = sc[src];
+}
+
 static nms_status amplitudes_common(nms_ctx* c, const nms_qgrid* grid, bool split, const int32_t* kinds_dev, int n_kinds,
                                     int* n_chunks)
 {
     if (!c->packed_valid) return fail(c, NMS_E_STATE, "no sample: call nms_set_sample first");
     if (nms_status st = set_grid(c, grid)) return st;
+    c->friedel_active = false;
+    if (c->opt_friedel) {
+        if (split) return fail(c, NMS_E_UNSUPPORTED, "Friedel halving does not cover the form-factor split");
+        if (!friedel_admissible(c))
+            return fail(c, NMS_E_UNSUPPORTED, "Friedel halving needs a polar grid with an even number of angles closed under theta -> theta + pi");
+    }
     AmpPlan plan;
-    if (nms_status st = plan_amplitude(c, split, &plan)) return st;
-    if (nms_status st = launch_amplitude(c, plan, kinds_dev, n_kinds)) return st;
+    if (!c->opt_friedel) {
+        if (nms_status st = plan_amplitude(c, split, &plan)) return st;
+        if (nms_status st = launch_amplitude(c, plan, kinds_dev, n_kinds)) return st;
+    } else {
+        // run the amplitude kernels on the first half of every ring: the context describes the half grid for the launch
+        const int n1 = c->g_n1, hn = n1 / 2;
+        const int64_t nq = c->n_q;
+        if (nms_status st = ensure(c, c->qc_half, sizeof(double2) * (size_t)c->g_n0 * hn)) return st;
+        if (nms_status st = ensure(c, c->sc_half, sizeof(double2) * (size_t)c->g_n0 * hn)) return st;
+        k_half_rings<<<(unsigned)(((int64_t)c->g_n0 * hn + 255) / 256), 256, 0, c->stream>>>(
+            (const double2*)c->qc.p, (const double2*)c->sc.p, c->g_n0, n1, (double2*)c->qc_half.p, (double2*)c->sc_half.p);
+        c->launches += 1;
+        std::swap(c->qc, c->qc_half); std::swap(c->sc, c->sc_half);
+        c->g_n1 = hn; c->n_q = (int64_t)c->g_n0 * hn;
+        nms_status st = plan_amplitude(c, false, &plan);
+        if (!st) st = launch_amplitude(c, plan, kinds_dev, n_kinds);
+        std::swap(c->qc, c->qc_half); std::swap(c->sc, c->sc_half);
+        c->g_n1 = n1; c->n_q = nq;
+        if (st) return st;
+        c->friedel_active = true;
+    }
     *n_chunks = c->n_chunks_used;
     return NMS_OK;
 }
@@ -563,6 +612,7 @@ nms_status nms_set_option(nms_ctx* c, const char* key, int64_t value)
     else if (!strcmp(key, "chunks")) { if (value < 0) return fail(c, NMS_E_ARG, "chunks must be >= 0"); c->opt_chunks = (int)value; }
     else if (!strcmp(key, "bases")) { if (value < 0 || value > 4) return fail(c, NMS_E_ARG, "bases must be 0..4"); c->opt_bases = (int)value; }
     else if (!strcmp(key, "precision")) { if (value < 0 || value > 2) return fail(c, NMS_E_ARG, "precision must be 0, 1 or 2"); c->opt_precision = (int)value; }
+    else if (!strcmp(key, "friedel")) { if (value < 0 || value > 1) return fail(c, NMS_E_ARG, "friedel must be 0 or 1"); c->opt_friedel = (int)value; }
     else if (!strcmp(key, "uniform")) { c->opt_uniform = (int)value; }
     else if (!strcmp(key, "recurrence")) { if (value < 0 || value > 2) return fail(c, NMS_E_ARG, "recurrence must be 0, 1 or 2"); c->opt_rec3 = (int)value; }
     else if (!strcmp(key, "qt")) { if (value != 0 && value != 4 && value != 8 && value != 16) return fail(c, NMS_E_ARG, "qt must be 0, 4, 8 or 16"); c->opt_qt = (int)value; }

@@ -63,6 +63,9 @@ struct nms_ctx {
     int opt_qt = 0;        // 0 auto, else 4/8/16
     int opt_bases = 0;     // recurrence kernels: exactly evaluated points per 8 (0 auto = 2, else 1..4)
     int opt_precision = 0; // 0 auto = 1 fast (MUFU phasors), 2 accurate (polynomial phasors)
+    int opt_friedel = 0;   // f-4: 1 = evaluate half of every ring and take the other half as the conjugate (polar grids)
+    bool friedel_active = false;   // the partials of the last amplitude launch cover the first half of every ring only
+    nms::DevBuf qc_half, sc_half;  // detector constants of the half rings
     int opt_uniform = 0;   // 1: never use the block-uniform instantiations (testing)
     int opt_rec3 = 0;      // recurrence kernels: 0 auto, 1 rotations, 2 three-term recurrence
     int amp_timer = NMS_T_AMPLITUDE;   // timer class of the amplitude launch (-1: none, the caller times it)

@@ -1087,3 +1087,44 @@ def test_batched_fields_errors(nms, ctx):
     assert e.value.status == nms.NMS_E_ARG
     nms.nms_compute_batch(ctx, wl.grid, mb, [0], out, None)
     nms.nms_synchronize(ctx)
+
+
+@pytest.mark.parametrize("name,small,variant", [("C1", False, 0), ("C5", True, 1), ("C5", True, 2)])
+def test_friedel_halving(nms, ctx, oracle_mod, name, small, variant):
+    """f-4: with option "friedel" the sums run over the first half of every ring and the second half is the conjugate
+    (A(-q) = A(q)^*, Eq. 42-43): amplitudes within 1e-5 sum|w| and the positive kinds at the north_star criterion
+    against the oracle on the FULL grid (the float angles theta_j + pi are met within 2.4e-7 rad)."""
+    import torch
+    wl = ni.make_config(name, small=small)
+    kinds = [KI[k] for k in ("NUC", "MAG", "UNPOL", "PROJ", "SF", "PP", "MM", "PM", "MP")]
+    _upload(nms, ctx, wl)
+    nms.nms_set_option(ctx, "variant", variant)
+    nms.nms_set_option(ctx, "friedel", 1)
+    nq = wl.grid.n_q
+    amp = torch.empty((8, nq), dtype=torch.float32, device="cuda")
+    maps = torch.empty((len(kinds), nq), dtype=torch.float32, device="cuda")
+    maps2 = torch.empty_like(maps)
+    nms.nms_amplitudes(ctx, wl.grid, amp)
+    nms.nms_response(ctx, kinds, maps)
+    nms.nms_compute(ctx, wl.grid, kinds, maps2)
+    nms.nms_synchronize(ctx)
+    assert torch.equal(maps, maps2)
+    qy, qz, th = oracle_mod.grid_points(wl.grid)
+    A, wsum, M = _oracle_maps(oracle_mod, wl, qy, qz, th, kinds)
+    a_h = amp.cpu().numpy()
+    assert_amplitudes(a_h, A, wsum, "friedel")
+    assert_cross_sections(maps.cpu().numpy(), M, kinds, "friedel")
+    n0, n1 = wl.grid.n0, wl.grid.n1
+    a3 = a_h.reshape(8, n0, n1)
+    assert np.array_equal(a3[0::2, :, n1 // 2:], a3[0::2, :, :n1 // 2])          # the second half IS the conjugate
+    assert np.array_equal(a3[1::2, :, n1 // 2:], -a3[1::2, :, :n1 // 2])
+    # not admissible: odd number of angles, Cartesian detector, form-factor split
+    out = torch.empty((1, 7 * 9), dtype=torch.float32, device="cuda")
+    for bad in (ni.polar_grid(np.linspace(0.1, 1.0, 7), 9), ni.cartesian_grid(np.linspace(-1, 1, 7), np.linspace(-1, 1, 9))):
+        with pytest.raises(nms.NmsError) as e:
+            nms.nms_compute(ctx, bad, [0], out)
+        assert e.value.status == nms.NMS_E_UNSUPPORTED
+    nms.nms_set_option(ctx, "friedel", 0)
+    nms.nms_compute(ctx, wl.grid, kinds, maps2)
+    nms.nms_synchronize(ctx)
+    assert_cross_sections(maps2.cpu().numpy(), M, kinds, "friedel off again")

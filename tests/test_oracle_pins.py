@@ -794,3 +794,21 @@ def test_batched_fields_share_the_nuclear_amplitude_and_are_linear(oracle_mod):
             np.testing.assert_allclose(A[b, 3 + 2 * c], Rn[c] * A_nuc[1], rtol=0, atol=1e-12 * scale)
     A1 = oracle_mod.amplitudes_batch(pos, N, mb[1:2], R, qy, qz)                                      # (iv)
     assert np.array_equal(A1[0], oracle_mod.amplitudes(pos, N, mb[1], R, qy, qz))
+
+
+# --------------------------------------------------------------------------- f-4: Friedel symmetry
+def test_friedel_symmetry_of_real_weights(oracle_mod):
+    """Eq. 42-43 (L353-L356) with real N_j, m_j: A(-q) = A(q)^*, exactly; on a ring, theta -> theta + pi is -q (L183).
+    Consequences for the responses: the |.|^2-type kinds are even, the chiral one is odd (pinned in
+    test_chiral_symmetries); here the amplitude identity itself, at exactly negated q."""
+    rng = np.random.Generator(np.random.Philox(404))
+    W = 300
+    pos = rng.uniform(-20, 20, size=(W, 3)).astype(np.float32)
+    N = rng.normal(size=W).astype(np.float32)
+    m = rng.normal(size=(W, 3)).astype(np.float32)
+    R = ni.rotation_alpha_beta(12.0, 77.0)
+    qy, qz = rng.uniform(-2, 2, size=50), rng.uniform(-2, 2, size=50)
+    A = oracle_mod.amplitudes(pos, N, m, R, qy, qz)
+    B = oracle_mod.amplitudes(pos, N, m, R, -qy, -qz)
+    np.testing.assert_allclose(B[0::2], A[0::2], rtol=0, atol=1e-12 * np.abs(A).max())
+    np.testing.assert_allclose(B[1::2], -A[1::2], rtol=0, atol=1e-12 * np.abs(A).max())
