@@ -166,7 +166,7 @@ nms_status plan_amplitude(nms_ctx* c, bool split, AmpPlan* plan)
     // the roofline against 2 bases + rotations, errors of the same size); the accurate variant keeps the rotations
     if (rec) {
         p.nb = c->opt_bases ? c->opt_bases : (p.qt == 16 ? 4 : (p.nch == 1 ? 2 : 1));
-        p.rec3 = c->opt_rec3 ? (c->opt_rec3 == 2) : (p.qt == 8 && !accurate && p.nb <= 2);
+        p.rec3 = c->opt_rec3 ? (c->opt_rec3 == 2) : (!accurate && (p.qt == 16 || p.nb <= 2));
         p.npoly = accurate ? 1 : 0;
         if (p.rec3 && p.qt == 8 && p.nb > 2) return fail(c, NMS_E_ARG, "the three-term recurrence needs bases <= 2");
     } else if (p.variant != 8) {
