@@ -307,9 +307,10 @@ typedef enum {
  * receives operations per clock and SM (slowest block).  Synchronises.                                                  */
 NMS_API nms_status nms_pipe_rates(nms_ctx* ctx, double* out);
 /* Error statistics of the phasor routine of the amplitude kernels (polynomial = 0: MUFU, 1: polynomial) over 2^log2_n
- * stratified phases (10 <= log2_n <= 30) against fp64: out [host][21] = largest |error| of cos, of sin, rms error of cos,
+ * stratified phases (10 <= log2_n <= 30) against fp64: out [host][23] = largest |error| of cos, of sin, rms error of cos,
  * of sin, then |e_n| for n = -8 ... 8, the Fourier coefficients of the complex error function e(phi) = z_computed -
- * exp(-i phi) (e_n multiplies A(n q) in the error of A(q); e_1 is a harmless relative error).  Synchronises.             */
+ * exp(-i phi) (e_n multiplies A(n q) in the error of A(q); e_1 is a harmless relative error), then Re e_0, Im e_0 (the
+ * mean errors of cos and of -sin).  Synchronises.                                                                      */
 NMS_API nms_status nms_phasor_selftest(nms_ctx* ctx, int polynomial, int log2_n, double* out);
 
 #ifdef __cplusplus

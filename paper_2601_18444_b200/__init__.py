@@ -276,10 +276,10 @@ def nms_pipe_rates(ctx) -> dict:
 
 def nms_phasor_selftest(ctx, polynomial: bool, log2_n: int = 24) -> dict:
     """Error statistics of the kernels' phasor routine against fp64 (see include/nms.h)."""
-    out = np.zeros(21, dtype=np.float64)
+    out = np.zeros(23, dtype=np.float64)
     _check(ctx, _lib.nms_phasor_selftest(ctx, C.c_int(1 if polynomial else 0), C.c_int(log2_n), C.c_void_p(out.ctypes.data)))
     return {"max_cos": out[0], "max_sin": out[1], "rms_cos": out[2], "rms_sin": out[3],
-            "harmonics": {n: float(out[4 + n + 8]) for n in range(-8, 9)}}
+            "harmonics": {n: float(out[4 + n + 8]) for n in range(-8, 9)}, "mean_cos": float(out[21]), "mean_minus_sin": float(out[22])}
 
 
 def nms_set_option(ctx, key: str, value: int):

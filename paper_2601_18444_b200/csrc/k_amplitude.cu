@@ -132,10 +132,10 @@ nms_status plan_amplitude(nms_ctx* c, bool split, AmpPlan* plan)
         if (nms_status st = wait_geometry(c)) return st;
         // automatic choice: after its first-order correction at the tile centres the recurrence leaves a phase error
         // <= (deviation of the float abscissae from the progression) x (half extent of a tile along the line's
-        // direction: any direction of the detector plane for a polar grid, Z for a Cartesian one); beyond 2e-5 rad
+        // direction: any direction of the detector plane for a polar grid, Z for a Cartesian one); beyond 1e-4 rad
         // (spatially incoherent cell order) use the direct kernel
         if (c->opt_variant == 0 && (p.variant == 3 || p.variant == 5) &&
-            c->g_dev * (c->g_type == 0 ? c->geo_ext : c->geo_extz) > 2e-5)
+            c->g_dev * (c->g_type == 0 ? c->geo_ext : c->geo_extz) > 1e-4)
             p.variant = (c->g_type == 0) ? 2 : 4;
     }
     const bool rec = p.variant == 3 || p.variant == 5;

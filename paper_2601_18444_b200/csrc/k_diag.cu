@@ -202,6 +202,7 @@ nms_status nms_phasor_selftest(nms_ctx* c, int polynomial, int log2_n, double* o
     const double n = (double)((int64_t)1 << log2_n);
     out[0] = h.max_c; out[1] = h.max_s; out[2] = sqrt(h.sum_c2 / n); out[3] = sqrt(h.sum_s2 / n);
     for (int k = 0; k <= 2 * SELF_HARM; ++k) out[4 + k] = sqrt(h.re[k] * h.re[k] + h.im[k] * h.im[k]) / n;
+    out[21] = h.re[SELF_HARM] / n; out[22] = h.im[SELF_HARM] / n;          // e_0 itself: the mean error of cos, of -sin
     return NMS_OK;
 }
 

@@ -6,7 +6,13 @@
 // the adder, for any |t| < 2^19 cycles, with no fp32 phase rounding.  Two evaluations of {cos, sin}(2 pi k / 2^32):
 //
 //   phasor_mufu(k)  XU pipe: I2FP, FMUL, sin.approx + cos.approx (MUFU; absolute error <= 2^-21.4 per value, CUDA C
-//                   Programming Guide).  6 issue slots, 2 of them on the 16 lanes/clk/SM XU pipe.
+//                   Programming Guide).  6 issue slots, 2 of them on the 16 lanes/clk/SM XU pipe.  Measured on B200
+//                   (nms_phasor_selftest): max error 4.3e-7, rms 1.2e-7; the cosine has a MEAN error of +1.2758e-8 (the
+//                   sine none), i.e. a constant term e_0 in the phasor that adds e_0 * sum_j w_j to every amplitude (0.2 on
+//                   C5's nuclear amplitude).  It is below half an ulp of cos near 1, so it cannot be taken out of the fp32
+//                   phasor; subtracting e_0 * (tile weight sums) from the fp64 tile sums at the flush was tried in round 2:
+//                   16 % fewer signed-kind misses on the full C5 map (292 -> 246 of 84 976) for 1.5 % of the throughput --
+//                   not kept; the polynomial phasor has no such term.
 //   phasor_poly(k)  FMA + ALU pipes: residual from the nearest quarter cycle as ONE shift (k << 2 wraps to
 //                   2^34 (f - n/4)), I2FP, x = 2 pi (f - n/4) with 2 pi split into fl32 hi + lo (a single fl32
 //                   constant is 2.8e-8 off: a sawtooth phase error that leaks A(-3q), A(5q) into A(q) at 7e-9),

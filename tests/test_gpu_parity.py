@@ -1016,7 +1016,10 @@ def test_phasor_error_statistics(nms, ctx):
     assert max(poly["max_cos"], poly["max_sin"]) <= 1.2e-7
     assert max(poly["rms_cos"], poly["rms_sin"]) <= 3e-8
     assert all(v <= 2e-9 for n, v in poly["harmonics"].items())
-    assert mufu["harmonics"][0] <= 2e-8                       # no constant term: nothing of sum w leaks into A(q)
+    # the constant term of the MUFU error is the mean error of its cosine, 1.2758e-8 on B200 (it adds that times sum w to
+    # every amplitude: DESIGN.md section 7 counts it among the causes of the signed-kind misses of the fp32 kernels)
+    assert abs(mufu["mean_cos"] - 1.2758e-8) <= 3e-10 and abs(mufu["mean_minus_sin"]) <= 3e-10
+    assert abs(poly["mean_cos"]) <= 1e-10
 
 
 def test_pipe_rates_are_sane(nms, ctx):
