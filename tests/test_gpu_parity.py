@@ -429,6 +429,36 @@ def test_form_factor_split_small(nms, ctx, oracle_mod):
     report_signed_misses(misses)
 
 
+@pytest.mark.parametrize("gtype,n1", [(0, 40), (0, 128), (1, 37)])
+def test_form_factor_split_line_recurrence(nms, ctx, oracle_mod, gtype, n1):
+    """The per-particle instantiation of the line-recurrence kernels (equally spaced |q| or q_z): total and form of the
+    positive kinds; n1 = 128 also runs the block-uniform instantiation of the polar three-term kernel in nms_compute."""
+    import torch
+    wl = ni.config_c3(K=5, n_q=24, n_theta=n1)
+    grid = ni.polar_grid(np.linspace(0.02, 1.9, 24), n1) if gtype == 0 else \
+        ni.cartesian_grid(np.linspace(-1.6, 1.7, 24), np.linspace(-1.5, 1.5, n1))
+    kinds = [KI[k] for k in ("NUC", "MAG", "UNPOL", "PROJ", "SF")]
+    _upload(nms, ctx, wl)
+    qy, qz, th = oracle_mod.grid_points(grid)
+    tot_ref, form_ref = oracle_mod.form_factor_split(wl.pos, wl.N, wl.m, wl.offsets, kinds, qy, qz, th, R=wl.R,
+                                                     centres=wl.centres, P=wl.P)
+    tot = torch.empty((len(kinds), grid.n_q), dtype=torch.float32, device="cuda")
+    form = torch.empty_like(tot)
+    maps = torch.empty_like(tot)
+    for rec, prec in ((0, 0), (1, 0), (0, 2)):
+        nms.nms_set_option(ctx, "variant", 2)
+        nms.nms_set_option(ctx, "recurrence", rec)
+        nms.nms_set_option(ctx, "precision", prec)
+        nms.nms_form_factor_split(ctx, grid, kinds, tot, form)
+        nms.nms_synchronize(ctx)
+        assert nms.nms_get_info(ctx, "variant_used") == (3 if gtype == 0 else 5)
+        assert_cross_sections(tot.cpu().numpy(), tot_ref, kinds, f"split recurrence total {rec} {prec}")
+        assert_cross_sections(form.cpu().numpy(), form_ref, kinds, f"split recurrence form {rec} {prec}")
+        nms.nms_compute(ctx, grid, kinds, maps)
+        nms.nms_synchronize(ctx)
+        assert_cross_sections(maps.cpu().numpy(), tot_ref, kinds, f"recurrence ordinary total {rec} {prec}")
+
+
 def test_form_factor_split_uneven_objects(nms, ctx, oracle_mod):
     """Objects of very different sizes (1 cell .. > 1 tile), one of them empty."""
     import torch
