@@ -267,6 +267,7 @@ NMS_API nms_status nms_get_weight_sums(nms_ctx* ctx, double* out);
  * for the first half of every ring only and the second half is taken as the conjugate, A(-q) = A(q)^* for real weights
  * (Eq. 42-43): half the pair evaluations; the second half then belongs to the float angle rotated by
  * its deviation from theta + pi (<= 2.4e-7 rad).  Off by default; bench.py reports it as an EFFECTIVE rate only.
+ * "uniform": 1 = do not use the block-uniform instantiation of the polar recurrence kernel (testing).
  * Unknown keys: NMS_E_ARG.  The fp32 kernels need q_max r_max / 2 pi < 2^19 cycles (NMS_E_UNSUPPORTED
  * otherwise; the exact kernel has no such limit).                                                        */
 NMS_API nms_status nms_set_option(nms_ctx* ctx, const char* key, int64_t value);

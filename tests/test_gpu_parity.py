@@ -1161,3 +1161,32 @@ def test_friedel_halving(nms, ctx, oracle_mod, name, small, variant):
     nms.nms_compute(ctx, wl.grid, kinds, maps2)
     nms.nms_synchronize(ctx)
     assert_cross_sections(maps2.cpu().numpy(), M, kinds, "friedel off again")
+
+
+def test_run_host_split_and_scan_match_device_path(nms, ctx):
+    """The one-call host entry points of the per-particle split (C3's e2e arm) and of the rocking scan (C4's) give the
+    maps of the device-resident call sequence bit for bit."""
+    import torch
+    w3 = ni.config_c3(K=7, n_q=21, n_theta=40, separate_centres=True)
+    k3 = w3.kinds
+    nq = w3.grid.n_q
+    h_tot = np.empty((len(k3), nq), dtype=np.float32)
+    h_form = np.empty_like(h_tot)
+    nms.nms_run_host_split(ctx, w3.pos, w3.N, w3.m, w3.offsets, w3.centres, w3.R, w3.grid, k3, h_tot, h_form)
+    _upload(nms, ctx, w3)
+    tot = torch.empty((len(k3), nq), dtype=torch.float32, device="cuda")
+    form = torch.empty_like(tot)
+    nms.nms_form_factor_split(ctx, w3.grid, k3, tot, form)
+    nms.nms_synchronize(ctx)
+    assert np.array_equal(tot.cpu().numpy(), h_tot) and np.array_equal(form.cpu().numpy(), h_form)
+    w4 = ni.make_config("C4", small=True)
+    k4, nq4 = w4.kinds, w4.grid.n_q
+    h_scan = np.empty((len(w4.rotations), len(k4), nq4), dtype=np.float32)
+    nms.nms_run_host_scan(ctx, w4.pos, w4.N, w4.m, w4.rotations, w4.grid, k4, h_scan)
+    nms.nms_set_sample(ctx, _t(w4.pos), _t(w4.N), _t(w4.m), w4.rotations[0])
+    maps = torch.empty((len(k4), nq4), dtype=torch.float32, device="cuda")
+    for i, R in enumerate(w4.rotations):
+        nms.nms_set_rotation(ctx, R)
+        nms.nms_compute(ctx, w4.grid, k4, maps)
+        nms.nms_synchronize(ctx)
+        assert np.array_equal(maps.cpu().numpy(), h_scan[i]), f"rotation {i}"
