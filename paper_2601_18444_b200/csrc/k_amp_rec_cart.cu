@@ -13,8 +13,13 @@ static amp_kernel_t pick(bool split, bool poly)
     return poly ? (amp_kernel_t)k_amp<1, QT, false, 4, NB, NCH, 1, REC3> : (amp_kernel_t)k_amp<1, QT, false, 4, NB, NCH, 0, REC3>;
 }
 
-amp_kernel_t amp_kernel_rec_cart(int qt, int nb, bool split, int nch, bool poly, bool rec3, bool uni)
+amp_kernel_t amp_kernel_rec_cart(int qt, int nb, bool split, int nch, bool poly, bool rec3, bool uni, bool sh)
 {
+    // accurate variant with a step phase within a quarter cycle: rotations (the default of precision 2) or three-term
+    if (sh && poly && qt == 8 && nb == 1 && nch == 4) {
+        if (rec3) return split ? (amp_kernel_t)k_amp<1, 8, true, 4, 1, 4, 1, 1, false, true> : (amp_kernel_t)k_amp<1, 8, false, 4, 1, 4, 1, 1, false, true>;
+        return split ? (amp_kernel_t)k_amp<1, 8, true, 4, 1, 4, 1, 0, false, true> : (amp_kernel_t)k_amp<1, 8, false, 4, 1, 4, 1, 0, false, true>;
+    }
     (void)uni;   // no gain measured on Cartesian lines (C4: 0.8136 against 0.8120)
     if (nch == 1) {
         if (split) return nullptr;

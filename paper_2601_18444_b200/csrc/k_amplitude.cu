@@ -61,8 +61,8 @@ static amp_kernel_t pick_kernel(const AmpPlan& p)
     case 1: return amp_kernel_direct(2, p.qt, p.split, p.nch, p.npoly, false);
     case 2: return amp_kernel_direct(0, p.qt, p.split, p.nch, p.npoly, p.uni);
     case 4: return amp_kernel_direct(1, p.qt, p.split, p.nch, p.npoly, p.uni);
-    case 3: return amp_kernel_rec_polar(p.qt, p.nb, p.split, p.nch, p.npoly != 0, p.rec3 != 0, p.uni);
-    case 5: return amp_kernel_rec_cart(p.qt, p.nb, p.split, p.nch, p.npoly != 0, p.rec3 != 0, p.uni);
+    case 3: return amp_kernel_rec_polar(p.qt, p.nb, p.split, p.nch, p.npoly != 0, p.rec3 != 0, p.uni, p.sh);
+    case 5: return amp_kernel_rec_cart(p.qt, p.nb, p.split, p.nch, p.npoly != 0, p.rec3 != 0, p.uni, p.sh);
     default: return p.split ? (amp_kernel_t)k_amp_f64<true> : (amp_kernel_t)k_amp_f64<false>;
     }
 }
@@ -173,10 +173,11 @@ nms_status plan_amplitude(nms_ctx* c, bool split, AmpPlan* plan)
         p.npoly = accurate ? p.qt : 0;
     }
     p.uni = c->g_n1 % AMP_THREADS == 0 && c->opt_uniform != 1;
+    p.sh = rec && accurate && fabs(c->g_dq) * c->geo_rmax < 0.24 * 6.283185307179586 && c->opt_uniform != 1;
     amp_kernel_t kern = pick_kernel(p);
     if (!kern) return fail(c, NMS_E_ARG, "no amplitude kernel for variant %d qt %d bases %d polynomial %d three-term %d",
                            p.variant, p.qt, p.nb, p.npoly, p.rec3);
-    const size_t smem = p.variant == 8 ? 0 : amp_smem_bytes(p.qt, p.nch, split);
+    const size_t smem = p.variant == 8 ? 0 : amp_smem_bytes(p.qt, p.nch, split, p.npoly != 0 && !split);
     NMS_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int occ = 0;
     NMS_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, AMP_THREADS, smem));
@@ -231,7 +232,7 @@ nms_status launch_amplitude(nms_ctx* c, const AmpPlan& plan, const int32_t* kind
     a.rp.Px = c->P[0]; a.rp.Py = c->P[1]; a.rp.Pz = c->P[2]; a.rp.sN = c->sN; a.rp.sM = c->sM; a.rp.invV = c->invV;
 
     amp_kernel_t kern = pick_kernel(plan);
-    const size_t smem = plan.variant == 8 ? 0 : amp_smem_bytes(plan.qt, plan.nch, plan.split);
+    const size_t smem = plan.variant == 8 ? 0 : amp_smem_bytes(plan.qt, plan.nch, plan.split, plan.npoly != 0 && !plan.split);
     NMS_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     dim3 grid((unsigned)plan.n_qblocks, (unsigned)n_chunks);
     // the kernels accumulate into their chunk partials with reductions

@@ -73,9 +73,12 @@ typedef void (*amp_kernel_t)(const AmpArgs);
 // shared memory of the fp32 kernels: two tile stages, two mbarriers, and in split mode the fp32 running
 // amplitudes of the current object (QT * 2 * NCH floats per thread)
 constexpr size_t AMP_SMEM_TILES = 2 * STAGE_CELLS * sizeof(Cell) + 2 * sizeof(uint64_t);
-constexpr size_t amp_smem_bytes(int qt, int nch, bool split)
+// ... and in the accurate non-split kernels the fp64 sub-accumulators of the nuclear channel (QT * 2 doubles per thread)
+constexpr int NSUB_CELLS = 16;
+constexpr size_t amp_smem_bytes(int qt, int nch, bool split, bool nsub)
 {
-    return AMP_SMEM_TILES + (split ? (size_t)qt * 2 * nch * AMP_THREADS * sizeof(float) : 0);
+    return AMP_SMEM_TILES + (split ? (size_t)qt * 2 * nch * AMP_THREADS * sizeof(float) : 0) +
+           (nsub ? (size_t)qt * 2 * AMP_THREADS * sizeof(double) : 0);
 }
 
 // ---- mbarrier / bulk-copy primitives (sm_90+ PTX) ----------------------------------------------
@@ -194,7 +197,9 @@ template <int QT, int NB> struct Seg {
 //         REC3 = 1: three-term recurrence instead of rotations.
 // UNI: the launch guarantees n1 % 128 == 0, so a block lies inside ONE group of QT lines: the line abscissae are then
 //      block-uniform values (derived from blockIdx only), which frees the 2 QT registers a thread needs for them.
-template <int MODE, int QT, bool SPLIT, int MINB, int NB, int NCH, int NPOLY, int REC3, bool UNI = false>
+// SH:  polynomial recurrence kernels only: the step phase stays within a quarter cycle (checked on the host: d r_max <
+//      pi / 2), so the step phasor needs no quadrant logic (sincos_poly_half).
+template <int MODE, int QT, bool SPLIT, int MINB, int NB, int NCH, int NPOLY, int REC3, bool UNI = false, bool SH = false>
 __global__ void __launch_bounds__(AMP_THREADS, MINB) k_amp(const AmpArgs a)
 {
     static_assert(NB == 0 || (MODE != 2 && NB <= QT), "the recurrence needs a line of equally spaced abscissae");
@@ -202,6 +207,13 @@ __global__ void __launch_bounds__(AMP_THREADS, MINB) k_amp(const AmpArgs a)
     Cell* sC = reinterpret_cast<Cell*>(smem_raw);                                          // [2][STAGE_CELLS]
     uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + 2 * STAGE_CELLS * sizeof(Cell));
     float* obj = reinterpret_cast<float*>(smem_raw + AMP_SMEM_TILES);                       // split: [QT*2*NCH][128]
+    // Accurate variant (polynomial phasors), nuclear channel: its weights are typically uniform (N_j = const inside the
+    // sample), so a tile whose cells share one phase (an x-row of a lattice: q_x = 0) adds the SAME number 256 times and
+    // the fp32 roundings drift instead of averaging out (measured: rms error of C5's nuclear amplitude 0.14 against 0.011
+    // with fp64 accumulation -- all of the remaining north-star misses of NM).  Every NSUB_CELLS cells the nuclear
+    // accumulators are therefore moved into fp64 sums in shared memory.
+    constexpr bool NSUB = NPOLY != 0 && !SPLIT;
+    double* nacc = reinterpret_cast<double*>(smem_raw + AMP_SMEM_TILES);                    // NSUB: [QT*2][128]
 
     const int tid = threadIdx.x;
     const int chunk = blockIdx.y;
@@ -290,8 +302,7 @@ __global__ void __launch_bounds__(AMP_THREADS, MINB) k_amp(const AmpArgs a)
         mbar_wait(&bar[stage], (uint32_t)((it >> 1) & 1));
 
         const int nc = tm.n_slots;
-#pragma unroll 8
-        for (int j = 0; j < nc; ++j) {
+        auto cell = [&](int j) {
             const double2 YZ = *reinterpret_cast<const double2*>(&tC[j].Y);
             const float4 w = *reinterpret_cast<const float4*>(&tC[j].wN);
             double p = 0.0;
@@ -310,7 +321,8 @@ __global__ void __launch_bounds__(AMP_THREADS, MINB) k_amp(const AmpArgs a)
             } else {
                 // step phasor of this cell: phase step dq' p (polar) or dq' Z (Cartesian), exactly reduced
                 float cd, sd;
-                unpack2(phasor<(NPOLY != 0)>(fma(dq, MODE == 0 ? p : YZ.y, MAGIC)), cd, sd);
+                if (SH) sincos_poly_half(__double2loint(fma(dq, MODE == 0 ? p : YZ.y, MAGIC)), cd, sd);
+                else unpack2(phasor<(NPOLY != 0)>(fma(dq, MODE == 0 ? p : YZ.y, MAGIC)), cd, sd);
                 const float two_cd = cd + cd;
 #pragma unroll
                 for (int b = 0; b < NBX; ++b) {
@@ -332,6 +344,26 @@ __global__ void __launch_bounds__(AMP_THREADS, MINB) k_amp(const AmpArgs a)
             }
 #pragma unroll
             for (int k = 0; k < QT; ++k) accumulate<NCH>(acc[k], w, ph[k]);
+        };
+        if (!NSUB) {
+#pragma unroll 8
+            for (int j = 0; j < nc; ++j) cell(j);
+        } else {
+#pragma unroll
+            for (int r = 0; r < 2 * QT; ++r) nacc[r * AMP_THREADS + tid] = 0.0;
+            for (int j0 = 0; j0 < nc; j0 += NSUB_CELLS) {
+                const int j1 = min(nc, j0 + NSUB_CELLS);
+#pragma unroll 8
+                for (int j = j0; j < j1; ++j) cell(j);
+#pragma unroll
+                for (int k = 0; k < QT; ++k) {
+                    float cs, sn;
+                    unpack2(acc[k][0], cs, sn);
+                    nacc[(2 * k) * AMP_THREADS + tid] += (double)cs;
+                    nacc[(2 * k + 1) * AMP_THREADS + tid] += (double)sn;
+                    acc[k][0] = 0ull;
+                }
+            }
         }
 
         __syncthreads();   // every thread is done with this stage: refill it while the flush runs
@@ -358,6 +390,12 @@ __global__ void __launch_bounds__(AMP_THREADS, MINB) k_amp(const AmpArgs a)
 #pragma unroll
                     for (int w = 0; w < 4; ++w) {
                         float cs = 0.f, sn = 0.f;
+                        if (NSUB && w == 0) {              // the nuclear tile sums are the fp64 sub-accumulators
+                            const double dc = nacc[(2 * k) * AMP_THREADS + tid], ds = nacc[(2 * k + 1) * AMP_THREADS + tid];
+                            Ap[0] = fma(-(double)eps, ds, dc);
+                            Ap[1] = -fma((double)eps, dc, ds);
+                            continue;
+                        }
                         if (w < NCH) {
                             unpack2(acc[k][w % NCH], cs, sn);
                             if (NB > 0) {                  // cos(psi + eps), sin(psi + eps) to first order
@@ -390,7 +428,7 @@ __global__ void __launch_bounds__(AMP_THREADS, MINB) k_amp(const AmpArgs a)
 
 // lookup functions of the three instantiation units (NULL if the combination is not built)
 amp_kernel_t amp_kernel_direct(int mode, int qt, bool split, int nch, int npoly, bool uni);
-amp_kernel_t amp_kernel_rec_polar(int qt, int nb, bool split, int nch, bool poly, bool rec3, bool uni);
-amp_kernel_t amp_kernel_rec_cart(int qt, int nb, bool split, int nch, bool poly, bool rec3, bool uni);
+amp_kernel_t amp_kernel_rec_polar(int qt, int nb, bool split, int nch, bool poly, bool rec3, bool uni, bool sh);
+amp_kernel_t amp_kernel_rec_cart(int qt, int nb, bool split, int nch, bool poly, bool rec3, bool uni, bool sh);
 
 }  // namespace nms

@@ -157,6 +157,7 @@ struct AmpPlan {
     int npoly;         // direct: phasors per thread evaluated by polynomial (qt = all: accurate); recurrence: 0 / 1
     int nb;            // recurrence: exactly evaluated points per thread
     int rec3;          // recurrence: three-term recurrence instead of rotations
+    bool sh;           // accurate recurrence: the step phase stays within a quarter cycle (no quadrant logic)
     bool uni;          // n1 % 128 == 0: a block lies inside one group of lines (block-uniform abscissae)
 };
 nms_status plan_amplitude(nms_ctx* c, bool split, AmpPlan* plan);

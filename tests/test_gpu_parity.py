@@ -302,18 +302,30 @@ def test_full_size_sampled(nms, ctx, oracle_mod, name, n_sample):
     report_signed_misses(misses)
 
 
-def test_c5_full_map_end_to_end(nms, ctx, oracle_mod):
-    """C5 at full size through the call sequence bench.py times (nms_compute, ring average, c(r), p(r)) against the
-    FULL fp64 map of the oracle (exact x-collapse, tests/c5_reference.py): amplitudes-free comparison of all 13 maps at
-    every one of the 262 144 detector points, the 512-ring I(q) (Eq. 30) and c(r), p(r) at 1024 r (Eq. 34-35
-    L205-L207).  The oracle side takes 1-3 minutes on the box's cores."""
-    import torch
+@pytest.fixture(scope="module")
+def c5_full(oracle_mod):
+    """The workload C5 and its full-map fp64 reference (exact x-collapse, tests/c5_reference.py); 1-3 minutes of CPU."""
     import c5_reference
     wl = ni.make_config("C5")
-    kinds = wl.kinds
     A, wsum, th = c5_reference.full_reference(oracle_mod, wl)
+    return wl, A, wsum, th
+
+
+@pytest.mark.parametrize("precision", [0, 2])
+def test_c5_full_map_end_to_end(nms, ctx, oracle_mod, c5_full, precision):
+    """C5 at full size through the call sequence bench.py times (nms_compute, ring average, c(r), p(r)) against the
+    FULL fp64 map of the oracle: all 13 maps at every one of the 262 144 detector points, the amplitudes, the 512-ring
+    I(q) (Eq. 30) and c(r), p(r) at 1024 r (Eq. 34-35).
+    precision 0: the default kernel (three-term line recurrence, MUFU phasors) -- the configuration of the headline bench
+    line; a miss of NM / CHI is reported as xfail.  precision 2: the accurate variant (polynomial
+    phasors, rotations, fp64 sub-accumulation of the nuclear channel) -- every kind, NM and CHI included, must meet the
+    north_star criterion at every point."""
+    import torch
+    wl, A, wsum, th = c5_full
+    kinds = wl.kinds
     M = oracle_mod.response(A, th, kinds, P=wl.P)
     _upload(nms, ctx, wl)
+    nms.nms_set_option(ctx, "precision", precision)
     nq, nb, nr, nk = wl.grid.n_q, wl.n_bins, len(wl.r), len(kinds)
     f32 = dict(dtype=torch.float32, device="cuda")
     maps, I, qb = torch.empty((nk, nq), **f32), torch.empty((nk, nb), **f32), torch.empty(nb, **f32)
@@ -326,9 +338,10 @@ def test_c5_full_map_end_to_end(nms, ctx, oracle_mod):
     nms.nms_amplitudes(ctx, wl.grid, amp)
     nms.nms_synchronize(ctx)
     assert nms.nms_get_info(ctx, "variant_used") == 3
+    assert (nms.nms_get_info(ctx, "poly_phasors") != 0) == (precision == 2)
     np.testing.assert_allclose(nms.nms_get_weight_sums(ctx), wsum, rtol=1e-12)
     assert_amplitudes(amp.cpu().numpy(), A, wsum, "C5 full map")
-    misses = []
+    misses = [] if precision == 0 else None
     assert_cross_sections(maps.cpu().numpy(), M, kinds, "C5 full map", signed_misses=misses)
     # 1-D outputs.  north_star states a criterion for the 2-D cross sections only; what it implies for a ring mean and
     # for its Fourier-Bessel transform follows by the triangle inequality: maps within 1e-3
