@@ -80,6 +80,7 @@ int choose_chunks(nms_ctx* c, int64_t n_qb, int64_t slots, int64_t units, double
     const int64_t mem_cap = (int64_t)(2.0e9 / chunk_bytes);
     if (max_chunks > mem_cap) max_chunks = mem_cap < 1 ? 1 : mem_cap;
     if (max_chunks > 4096) max_chunks = 4096;
+    if (n_qb * (units / min_units) < 2 * slots) min_units = 1;   // small problem: filling the device comes first
     if (max_chunks > units / min_units) max_chunks = units / min_units < 1 ? 1 : units / min_units;
     int64_t best_c = 1; double best_eff = -1.0;
     if (c->opt_chunks > 0) return (int)(c->opt_chunks < units ? c->opt_chunks : units);
