@@ -73,11 +73,11 @@ static int64_t ceil_div(int64_t a, int64_t b) { return (a + b - 1) / b; }
 // C4 0.763 -> 0.813, C3 0.587 -> 0.630 of the roofline from 9 chunks to 16+ waves) -- the blocks are equal-sized, so
 // what counts is that blocks / (SMs x resident blocks) comes out close to a whole number and that there are enough
 // waves for the dynamic scheduler to even out.  Search 16 ... 48 waves for the best product of wave fill and unit
-// balance; the fp64 partials (chunk_bytes per chunk) cap it at 2 GB; at least min_units units of work per chunk.
-int choose_chunks(nms_ctx* c, int64_t n_qb, int64_t slots, int64_t units, double chunk_bytes, int64_t min_units)
+// balance; the fp64 partials (chunk_bytes per chunk) cap it at mem_bytes; at least min_units units of work per chunk.
+int choose_chunks(nms_ctx* c, int64_t n_qb, int64_t slots, int64_t units, double chunk_bytes, int64_t min_units, double mem_bytes)
 {
     int64_t max_chunks = units;
-    const int64_t mem_cap = (int64_t)(2.0e9 / chunk_bytes);
+    const int64_t mem_cap = (int64_t)(mem_bytes / chunk_bytes);
     if (max_chunks > mem_cap) max_chunks = mem_cap < 1 ? 1 : mem_cap;
     if (max_chunks > 4096) max_chunks = 4096;
     if (n_qb * (units / min_units) < 2 * slots) min_units = 1;   // small problem: filling the device comes first
@@ -113,18 +113,20 @@ nms_status wait_geometry(nms_ctx* c)
     return NMS_OK;
 }
 
-nms_status plan_amplitude(nms_ctx* c, bool split, AmpPlan* plan)
+nms_status plan_amplitude(nms_ctx* c, bool split, bool want_accurate, AmpPlan* plan)
 {
     // precision policy: small problems run the exact fp64 kernel; otherwise the line
-    // recurrence where the thread lines are equally spaced, else the direct kernel; MUFU phasors unless the
-    // "precision" option asks for the polynomial ones
+    // recurrence where the thread lines are equally spaced, else the direct kernel.  The accurate variant (polynomial
+    // phasors, rotations, fp64 sub-accumulation of the nuclear channel) runs when the caller needs the signed kinds NM /
+    // CHI at the north-star criterion (want_accurate: they were requested, or the amplitudes are kept for later requests),
+    // the fast one (MUFU phasors, three-term recurrence) otherwise; the "precision" option overrides: 1 fast, 2 accurate
     AmpPlan p = {};
     p.split = split;
     const bool small = (double)c->W * (double)c->n_q <= 1073741824.0;
     const bool line_ok = c->g_type != 2 && c->g_uniform && c->g_n0 >= 2;
     if (c->opt_variant == 2 && !line_ok)
         return fail(c, NMS_E_UNSUPPORTED, "the line-recurrence variant needs a polar or Cartesian detector with equally spaced u0");
-    const bool accurate = c->opt_precision == 2;
+    const bool accurate = c->opt_precision == 2 || (c->opt_precision == 0 && want_accurate);
     if (c->opt_variant == 3 || (c->opt_variant == 0 && small)) p.variant = 8;
     else if (c->g_type == 2) p.variant = 1;
     else if (c->opt_variant == 2 || (c->opt_variant == 0 && line_ok)) p.variant = (c->g_type == 0) ? 3 : 5;
@@ -187,7 +189,11 @@ nms_status plan_amplitude(nms_ctx* c, bool split, AmpPlan* plan)
     const int64_t n_qb = p.variant == 8 ? ceil_div(c->n_q, AMP_THREADS)
                                         : ceil_div(ceil_div(c->g_n0, p.qt) * c->g_n1, AMP_THREADS);
 
-    p.n_chunks = choose_chunks(c, n_qb, slots, units, 8.0 * (double)c->n_q * (split ? 8.0 + NMS_KIND_COUNT : 8.0), split ? 1 : 8);
+    // per-particle split: every object's flush adds to (8 + n_kinds) planes of its chunk -- keep those within 0.3 GB so that
+    // they are written to DRAM once, not once per object (C3: 46 chunks instead of 148 cost 1 % and cut the kernel's DRAM
+    // writes from 1.96 GB to under 0.6 GB)
+    p.n_chunks = choose_chunks(c, n_qb, slots, units, 8.0 * (double)c->n_q * (split ? 8.0 + NMS_KIND_COUNT : 8.0), split ? 1 : 8,
+                               split ? 0.3e9 * (8.0 + NMS_KIND_COUNT) / 12.0 : 2.0e9);
     p.n_qblocks = (int)n_qb; p.blocks_per_sm = occ;
     *plan = p;
     return NMS_OK;

@@ -74,7 +74,7 @@ typedef void (*amp_kernel_t)(const AmpArgs);
 // amplitudes of the current object (QT * 2 * NCH floats per thread)
 constexpr size_t AMP_SMEM_TILES = 2 * STAGE_CELLS * sizeof(Cell) + 2 * sizeof(uint64_t);
 // ... and in the accurate non-split kernels the fp64 sub-accumulators of the nuclear channel (QT * 2 doubles per thread)
-constexpr int NSUB_CELLS = 16;
+constexpr int NSUB_CELLS = 32;   // 16: 0.552 of the roofline on C5, worst signed-kind error 6.7e-4; 32: 0.566, 7.3e-4
 constexpr size_t amp_smem_bytes(int qt, int nch, bool split, bool nsub)
 {
     return AMP_SMEM_TILES + (split ? (size_t)qt * 2 * nch * AMP_THREADS * sizeof(float) : 0) +

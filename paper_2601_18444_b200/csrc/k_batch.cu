@@ -87,12 +87,14 @@ constexpr size_t BATCH_SMEM = 2 * TILE * sizeof(BCell) + 2 * sizeof(uint64_t);
 // buffered), same exact phase reduction and MUFU phasor; 10 packed accumulations per pair.
 // 3 blocks per SM: 80 accumulator registers + phase constants need ~150 registers (at 128 the kernel spills and was
 // measured 20 % slower: C5 2578 against 3084 Gpair-field/s).
-template <int MODE>
+// ACC: the accurate variant (polynomial phasor, fp64 sub-accumulation of the shared nuclear channel every NSUB_CELLS cells).
+template <int MODE, bool ACC>
 __global__ void __launch_bounds__(AMP_THREADS, 3) k_amp_batch(const BatchArgs a)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     BCell* sC = reinterpret_cast<BCell*>(smem_raw);
     uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + 2 * TILE * sizeof(BCell));
+    double* nacc = reinterpret_cast<double*>(smem_raw + BATCH_SMEM);                       // ACC: [BQT * 2][128]
     const int tid = threadIdx.x, chunk = blockIdx.y;
     const int tile_beg = (int)(((int64_t)a.n_tiles * chunk) / gridDim.y);
     const int tile_end = (int)(((int64_t)a.n_tiles * (chunk + 1)) / gridDim.y);
@@ -146,8 +148,7 @@ __global__ void __launch_bounds__(AMP_THREADS, 3) k_amp_batch(const BatchArgs a)
 #pragma unroll
             for (int r = 0; r < BCH; ++r) acc[k][r] = 0ull;
         mbar_wait(&bar[stage], (uint32_t)((it >> 1) & 1));
-#pragma unroll 4
-        for (int j = 0; j < nc; ++j) {
+        auto cell = [&](int j) {
             const double2 YZ = *reinterpret_cast<const double2*>(&tC[j].Y);
             const float4 w0 = *reinterpret_cast<const float4*>(&tC[j].w[0]);
             const float4 w1 = *reinterpret_cast<const float4*>(&tC[j].w[4]);
@@ -161,7 +162,7 @@ __global__ void __launch_bounds__(AMP_THREADS, 3) k_amp_batch(const BatchArgs a)
                 if (MODE == 0) m = fma(g[k], p, MAGIC);
                 else if (MODE == 1) m = fma(g[k], YZ.y, p) + MAGIC;
                 else m = fma(g[k], YZ.y, h[k] * YZ.x) + MAGIC;
-                const u64 ph = phasor<false>(m);
+                const u64 ph = phasor<ACC>(m);
                 acc[k][0] = ffma2(pack2(w0.x, w0.x), ph, acc[k][0]);
                 acc[k][1] = ffma2(pack2(w0.y, w0.y), ph, acc[k][1]);
                 acc[k][2] = ffma2(pack2(w0.z, w0.z), ph, acc[k][2]);
@@ -172,6 +173,26 @@ __global__ void __launch_bounds__(AMP_THREADS, 3) k_amp_batch(const BatchArgs a)
                 acc[k][7] = ffma2(pack2(w1.w, w1.w), ph, acc[k][7]);
                 acc[k][8] = ffma2(pack2(w2.x, w2.x), ph, acc[k][8]);
                 acc[k][9] = ffma2(pack2(w2.y, w2.y), ph, acc[k][9]);
+            }
+        };
+        if (!ACC) {
+#pragma unroll 4
+            for (int j = 0; j < nc; ++j) cell(j);
+        } else {
+#pragma unroll
+            for (int r = 0; r < 2 * BQT; ++r) nacc[r * AMP_THREADS + tid] = 0.0;
+            for (int j0 = 0; j0 < nc; j0 += NSUB_CELLS) {
+                const int j1 = min(nc, j0 + NSUB_CELLS);
+#pragma unroll 4
+                for (int j = j0; j < j1; ++j) cell(j);
+#pragma unroll
+                for (int k = 0; k < BQT; ++k) {
+                    float cs, sn;
+                    unpack2(acc[k][0], cs, sn);
+                    nacc[(2 * k) * AMP_THREADS + tid] += (double)cs;
+                    nacc[(2 * k + 1) * AMP_THREADS + tid] += (double)sn;
+                    acc[k][0] = 0ull;
+                }
             }
         }
         __syncthreads();
@@ -184,8 +205,10 @@ __global__ void __launch_bounds__(AMP_THREADS, 3) k_amp_batch(const BatchArgs a)
                 for (int r = 0; r < BCH; ++r) {
                     float cs, sn;
                     unpack2(acc[k][r], cs, sn);
-                    atomicAdd(a.part + ((int64_t)chunk * 2 * BCH + 2 * r) * a.n_q + f, (double)cs);        // Re: + sum w cos
-                    atomicAdd(a.part + ((int64_t)chunk * 2 * BCH + 2 * r + 1) * a.n_q + f, -(double)sn);   // Im: - sum w sin
+                    double dc = (double)cs, ds = (double)sn;
+                    if (ACC && r == 0) { dc = nacc[(2 * k) * AMP_THREADS + tid]; ds = nacc[(2 * k + 1) * AMP_THREADS + tid]; }
+                    atomicAdd(a.part + ((int64_t)chunk * 2 * BCH + 2 * r) * a.n_q + f, dc);        // Re: + sum w cos
+                    atomicAdd(a.part + ((int64_t)chunk * 2 * BCH + 2 * r + 1) * a.n_q + f, -ds);   // Im: - sum w sin
                 }
             }
         }
@@ -227,17 +250,20 @@ __global__ void __launch_bounds__(256) k_epilogue_batch(const double* __restrict
 }
 
 nms_status launch_batch(nms_ctx* c, const float* m_batch, int B, const int32_t* kinds_dev, int n_kinds, float* out_maps,
-                        float* out_amp)
+                        float* out_amp, bool accurate)
 {
     if (nms_status st = wait_geometry(c)) return st;
     typedef void (*kern_t)(const BatchArgs);
-    kern_t kern = c->g_type == 0 ? (kern_t)k_amp_batch<0> : (c->g_type == 1 ? (kern_t)k_amp_batch<1> : (kern_t)k_amp_batch<2>);
-    NMS_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)BATCH_SMEM));
+    kern_t kern = c->g_type == 0 ? (kern_t)k_amp_batch<0, false> : (c->g_type == 1 ? (kern_t)k_amp_batch<1, false> : (kern_t)k_amp_batch<2, false>);
+    if (accurate)
+        kern = c->g_type == 0 ? (kern_t)k_amp_batch<0, true> : (c->g_type == 1 ? (kern_t)k_amp_batch<1, true> : (kern_t)k_amp_batch<2, true>);
+    const size_t smem = BATCH_SMEM + (accurate ? (size_t)BQT * 2 * AMP_THREADS * sizeof(double) : 0);
+    NMS_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int occ = 0;
-    NMS_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, AMP_THREADS, BATCH_SMEM));
+    NMS_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, AMP_THREADS, smem));
     if (occ < 1) return fail(c, NMS_E_CUDA, "batch amplitude kernel does not fit on an SM");
     const int64_t n_qb = (((int64_t)(c->g_n0 + BQT - 1) / BQT) * c->g_n1 + AMP_THREADS - 1) / AMP_THREADS;
-    const int n_chunks = choose_chunks(c, n_qb, (int64_t)c->sm_count * occ, c->n_tiles, 8.0 * 2 * BCH * (double)c->n_q, 8);
+    const int n_chunks = choose_chunks(c, n_qb, (int64_t)c->sm_count * occ, c->n_tiles, 8.0 * 2 * BCH * (double)c->n_q, 8, 2.0e9);
     const size_t part_bytes = sizeof(double) * 2 * BCH * (size_t)c->n_q * n_chunks;
     if (nms_status st = ensure(c, c->part, part_bytes)) return st;
     if (nms_status st = ensure(c, c->batch_cells, sizeof(BCell) * (size_t)c->n_slots)) return st;
@@ -270,7 +296,7 @@ nms_status launch_batch(nms_ctx* c, const float* m_batch, int B, const int32_t* 
         if (nms_status st = timer_end(c, NMS_T_PREP)) return st;
         NMS_CUDA(c, cudaMemsetAsync(c->part.p, 0, part_bytes, c->stream));
         if (nms_status st = timer_begin(c, NMS_T_BATCH)) return st;
-        kern<<<dim3((unsigned)n_qb, (unsigned)n_chunks), AMP_THREADS, BATCH_SMEM, c->stream>>>(a);
+        kern<<<dim3((unsigned)n_qb, (unsigned)n_chunks), AMP_THREADS, smem, c->stream>>>(a);
         if (nms_status st = timer_end(c, NMS_T_BATCH)) return st;
         if (nms_status st = timer_begin(c, NMS_T_EPILOGUE)) return st;
         k_epilogue_batch<<<(unsigned)((c->n_q + 255) / 256), 256, 0, c->stream>>>(
@@ -281,6 +307,7 @@ nms_status launch_batch(nms_ctx* c, const float* m_batch, int B, const int32_t* 
         NMS_CUDA(c, cudaGetLastError());
     }
     c->n_chunks_used = n_chunks; c->blocks_per_sm_used = occ; c->qt_used = BQT; c->variant_used = 16;
+    c->npoly_used = accurate ? BQT : 0; c->nb_used = 0; c->rec3_used = 0;
     return NMS_OK;
 }
 

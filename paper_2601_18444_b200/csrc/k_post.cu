@@ -322,7 +322,7 @@ nms_status launch_correlation_2d(nms_ctx* c, const float* map, const nms_qgrid* 
     exchange();                                   // the context now describes the pixel sample, no grid yet
     nms_status st = set_grid(c, rgrid);
     AmpPlan plan;
-    if (!st) st = plan_amplitude(c, false, &plan);
+    if (!st) st = plan_amplitude(c, false, false, &plan);
     if (!st) {
         st = timer_begin(c, NMS_T_CORR2D);
         if (!st) st = launch_amplitude(c, plan, nullptr, 0);

@@ -366,8 +366,18 @@ __global__ void k_half_rings(const double2* __restrict__ qc, const double2* __re
     sc_h[f] = sc[src];
 }
 
-static nms_status amplitudes_common(nms_ctx* c, const nms_qgrid* grid, bool split, const int32_t* kinds_dev, int n_kinds,
-                                    int* n_chunks)
+// The signed difference kinds NM = (PP - MM)/2 and CHI = (PM - MP)/2 cross zero; the north-star criterion (1e-3 relative
+// above 1e-6 of the map's own maximum) then asks the amplitudes for ~5e-10 sum|w|: they get the
+// accurate variant of the fp32 kernels unless the caller says otherwise.
+static bool wants_signed(const nms_kind* kinds, int n_kinds)
+{
+    for (int i = 0; i < n_kinds; ++i)
+        if (kinds[i] == NMS_NM || kinds[i] == NMS_CHI) return true;
+    return false;
+}
+
+static nms_status amplitudes_common(nms_ctx* c, const nms_qgrid* grid, bool split, bool want_accurate, const int32_t* kinds_dev,
+                                    int n_kinds, int* n_chunks)
 {
     if (!c->packed_valid) return fail(c, NMS_E_STATE, "no sample: call nms_set_sample first");
     if (nms_status st = set_grid(c, grid)) return st;
@@ -379,7 +389,7 @@ static nms_status amplitudes_common(nms_ctx* c, const nms_qgrid* grid, bool spli
     }
     AmpPlan plan;
     if (!c->opt_friedel) {
-        if (nms_status st = plan_amplitude(c, split, &plan)) return st;
+        if (nms_status st = plan_amplitude(c, split, want_accurate, &plan)) return st;
         if (nms_status st = launch_amplitude(c, plan, kinds_dev, n_kinds)) return st;
     } else {
         // run the amplitude kernels on the first half of every ring: the context describes the half grid for the launch
@@ -392,7 +402,7 @@ static nms_status amplitudes_common(nms_ctx* c, const nms_qgrid* grid, bool spli
         c->launches += 1;
         std::swap(c->qc, c->qc_half); std::swap(c->sc, c->sc_half);
         c->g_n1 = hn; c->n_q = (int64_t)c->g_n0 * hn;
-        nms_status st = plan_amplitude(c, false, &plan);
+        nms_status st = plan_amplitude(c, false, want_accurate, &plan);
         if (!st) st = launch_amplitude(c, plan, kinds_dev, n_kinds);
         std::swap(c->qc, c->qc_half); std::swap(c->sc, c->sc_half);
         c->g_n1 = n1; c->n_q = nq;
@@ -408,7 +418,7 @@ nms_status nms_amplitudes(nms_ctx* c, const nms_qgrid* grid, float* out_amp)
     CHECK_CTX(c);
     int n_chunks = 0;
     c->amp_valid = false;
-    if (nms_status st = amplitudes_common(c, grid, false, nullptr, 0, &n_chunks)) return st;
+    if (nms_status st = amplitudes_common(c, grid, false, true, nullptr, 0, &n_chunks)) return st;
     if (nms_status st = launch_epilogue(c, n_chunks, nullptr, 0, nullptr, out_amp, true)) return st;
     c->amp_valid = true;
     return NMS_OK;
@@ -440,7 +450,7 @@ nms_status nms_compute(nms_ctx* c, const nms_qgrid* grid, const nms_kind* kinds,
     if (nms_status st = upload_kinds(c, kinds, n_kinds, &kd)) return st;
     int n_chunks = 0;
     c->amp_valid = false;
-    if (nms_status st = amplitudes_common(c, grid, false, kd, n_kinds, &n_chunks)) return st;
+    if (nms_status st = amplitudes_common(c, grid, false, wants_signed(kinds, n_kinds), kd, n_kinds, &n_chunks)) return st;
     return launch_epilogue(c, n_chunks, kd, n_kinds, out, nullptr, false);
 }
 
@@ -456,7 +466,8 @@ nms_status nms_compute_batch(nms_ctx* c, const nms_qgrid* grid, const float* m_b
     if (nms_status st = upload_kinds(c, kinds, out_maps ? n_kinds : 0, &kd)) return st;
     if (nms_status st = set_grid(c, grid)) return st;
     c->amp_valid = false;
-    return launch_batch(c, m_batch, n_fields, kd, n_kinds, out_maps, out_amp);
+    const bool accurate = c->opt_precision == 2 || (c->opt_precision == 0 && (out_amp != nullptr || wants_signed(kinds, out_maps ? n_kinds : 0)));
+    return launch_batch(c, m_batch, n_fields, kd, n_kinds, out_maps, out_amp, accurate);
 }
 
 nms_status nms_form_factor_split(nms_ctx* c, const nms_qgrid* grid, const nms_kind* kinds, int n_kinds, float* out_total,
@@ -469,7 +480,7 @@ nms_status nms_form_factor_split(nms_ctx* c, const nms_qgrid* grid, const nms_ki
     if (nms_status st = upload_kinds(c, kinds, n_kinds, &kd)) return st;
     int n_chunks = 0;
     c->amp_valid = false;
-    if (nms_status st = amplitudes_common(c, grid, true, kd, n_kinds, &n_chunks)) return st;
+    if (nms_status st = amplitudes_common(c, grid, true, wants_signed(kinds, n_kinds), kd, n_kinds, &n_chunks)) return st;
     return launch_split_epilogue(c, n_chunks, kd, n_kinds, out_total, out_form);
 }
 

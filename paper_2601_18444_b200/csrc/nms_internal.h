@@ -62,7 +62,7 @@ struct nms_ctx {
     int opt_chunks = 0;
     int opt_qt = 0;        // 0 auto, else 4/8/16
     int opt_bases = 0;     // recurrence kernels: exactly evaluated points per 8 (0 auto = 2, else 1..4)
-    int opt_precision = 0; // 0 auto = 1 fast (MUFU phasors), 2 accurate (polynomial phasors)
+    int opt_precision = 0; // 0 auto (accurate where NM / CHI may be formed from the sums, else fast), 1 fast, 2 accurate
     int opt_friedel = 0;   // f-4: 1 = evaluate half of every ring and take the other half as the conjugate (polar grids)
     bool friedel_active = false;   // the partials of the last amplitude launch cover the first half of every ring only
     nms::DevBuf qc_half, sc_half;  // detector constants of the half rings
@@ -160,8 +160,8 @@ struct AmpPlan {
     bool sh;           // accurate recurrence: the step phase stays within a quarter cycle (no quadrant logic)
     bool uni;          // n1 % 128 == 0: a block lies inside one group of lines (block-uniform abscissae)
 };
-nms_status plan_amplitude(nms_ctx* c, bool split, AmpPlan* plan);
-int choose_chunks(nms_ctx* c, int64_t n_qb, int64_t slots, int64_t units, double chunk_bytes, int64_t min_units);
+nms_status plan_amplitude(nms_ctx* c, bool split, bool want_accurate, AmpPlan* plan);
+int choose_chunks(nms_ctx* c, int64_t n_qb, int64_t slots, int64_t units, double chunk_bytes, int64_t min_units, double mem_bytes);
 nms_status wait_geometry(nms_ctx* c);                     // r_max / tile extents of the packed sample (k_prep) on the host
 nms_status launch_amplitude(nms_ctx* c, const AmpPlan& plan, const int32_t* kinds_dev, int n_kinds);
 // k_epilogue.cu
@@ -173,7 +173,7 @@ nms_status launch_split_epilogue(nms_ctx* c, int n_chunks, const int32_t* kinds_
                                  float* out_form);
 // k_batch.cu
 nms_status launch_batch(nms_ctx* c, const float* m_batch, int B, const int32_t* kinds_dev, int n_kinds, float* out_maps,
-                        float* out_amp);
+                        float* out_amp, bool accurate);
 // k_post.cu
 nms_status launch_azimuthal(nms_ctx* c, const float* maps, int n_maps, int n_bins, double q_lo, double q_hi,
                             float* out_I, float* out_q, int32_t* out_count);

@@ -12,7 +12,9 @@
 //                   C5's nuclear amplitude).  It is below half an ulp of cos near 1, so it cannot be taken out of the fp32
 //                   phasor; subtracting e_0 * (tile weight sums) from the fp64 tile sums at the flush was tried in round 2:
 //                   16 % fewer signed-kind misses on the full C5 map (292 -> 246 of 84 976) for 1.5 % of the throughput --
-//                   not kept; the polynomial phasor has no such term.
+//                   not kept; the polynomial phasor has no such term.  The error is the MUFU tables' own: feeding the
+//                   unit a phase whose conversion is exact and rotating by the exactly known remainder (first order)
+//                   left max 3.5e-7 / rms 1e-7 unchanged (round-2 experiment).
 //   phasor_poly(k)  FMA + ALU pipes: residual from the nearest quarter cycle as ONE shift (k << 2 wraps to
 //                   2^34 (f - n/4)), I2FP, x = 2 pi (f - n/4) with 2 pi split into fl32 hi + lo (a single fl32
 //                   constant is 2.8e-8 off: a sawtooth phase error that leaks A(-3q), A(5q) into A(q) at 7e-9),

@@ -147,16 +147,17 @@ def _run_full(nms, h, wl, kinds):
 # C1, C2 at full size, full maps; every kernel variant the grid admits
 # ---------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("name", ["C1", "C2"])
-@pytest.mark.parametrize("variant,qt,bases,rec,prec", [(0, 0, 0, 0, 0), (3, 0, 0, 0, 0), (1, 0, 0, 0, 0), (1, 4, 0, 0, 0),
-                                                        (1, 8, 0, 0, 0), (1, 0, 0, 0, 2), (1, 4, 0, 0, 2),
-                                                        (2, 0, 0, 0, 0), (2, 0, 1, 1, 0), (2, 0, 2, 1, 0), (2, 0, 2, 2, 0),
-                                                        (2, 0, 3, 1, 0), (2, 0, 4, 1, 0), (2, 0, 0, 0, 2), (2, 0, 2, 2, 2)])
+@pytest.mark.parametrize("variant,qt,bases,rec,prec", [(0, 0, 0, 0, 0), (3, 0, 0, 0, 0), (1, 0, 0, 0, 1), (1, 4, 0, 0, 1),
+                                                        (1, 8, 0, 0, 1), (1, 0, 0, 0, 2), (1, 4, 0, 0, 0),
+                                                        (2, 0, 0, 0, 1), (2, 0, 1, 1, 1), (2, 0, 2, 1, 1), (2, 0, 2, 2, 1),
+                                                        (2, 0, 3, 1, 1), (2, 0, 4, 1, 1), (2, 0, 0, 0, 0), (2, 0, 2, 2, 2)])
 def test_full_config_maps(nms, ctx, oracle_mod, name, variant, qt, bases, rec, prec):
     """variant 0 = automatic (these small problems run the exact fp64 kernel), 3 = exact forced: every kind held to
     the north_star criterion.  1 = the fp32-accumulating direct kernels, 2 = the line-recurrence kernels with `bases`
-    exactly evaluated points per 8 by rotations (rec 1) or the three-term recurrence (rec 2), MUFU (prec 0) or
-    polynomial (prec 2) phasors: amplitudes and every kind to the same criterion; a miss of NM / CHI is reported as
-    xfail (C1 and C2 are below the size where the library itself would pick an fp32 kernel)."""
+    exactly evaluated points per 8 by rotations (rec 1) or the three-term recurrence (rec 2), MUFU (prec 1) or
+    polynomial (prec 2; prec 0 = automatic, which is 2 here: all 13 kinds are asked for) phasors: amplitudes and every
+    kind to the same criterion; a miss of NM / CHI is reported as xfail (C1 and C2 are below the size where the library
+    itself would pick an fp32 kernel)."""
     wl = ni.make_config(name)
     kinds = list(ni.ALL_KINDS)
     _upload(nms, ctx, wl)
@@ -176,10 +177,10 @@ def test_full_config_maps(nms, ctx, oracle_mod, name, variant, qt, bases, rec, p
     polar = wl.grid.type == 0
     assert used == {0: 8, 3: 8, 1: 2 if polar else 4, 2: 3 if polar else 5}[variant]
     if variant in (1, 2):
-        assert (nms.nms_get_info(ctx, "poly_phasors") != 0) == (prec == 2)
+        assert (nms.nms_get_info(ctx, "poly_phasors") != 0) == (prec != 1)
     if variant == 2:
         assert nms.nms_get_info(ctx, "bases") == (bases or 1)
-        assert nms.nms_get_info(ctx, "three_term") == (1 if rec == 2 or (rec == 0 and prec == 0) else 0)
+        assert nms.nms_get_info(ctx, "three_term") == (1 if rec == 2 or (rec == 0 and prec == 1) else 0)
     report_signed_misses(misses)
 
 
@@ -201,7 +202,7 @@ def test_c1_physics_on_gpu(nms, ctx):
 # reduced C3, C4, C5 (same structure, several tiles and a ragged tail), full maps
 # ---------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("name", ["C3", "C4", "C5"])
-@pytest.mark.parametrize("variant,prec", [(0, 0), (1, 0), (2, 0), (1, 2), (2, 2)])
+@pytest.mark.parametrize("variant,prec", [(0, 0), (1, 1), (2, 1), (1, 2), (2, 0)])
 def test_small_config_maps(nms, ctx, oracle_mod, name, variant, prec):
     """Every kernel family on the reduced configs, all 13 kinds at the north_star criterion (variant 0 picks the exact
     kernel at these sizes; a miss of NM / CHI by an fp32 kernel is reported as xfail)."""
@@ -246,17 +247,20 @@ def test_recurrence_ragged_lines(nms, ctx, oracle_mod, gtype, n0):
     nms.nms_set_option(ctx, "variant", 2 if n0 > 1 else 1)
     amp = torch.empty((8, grid.n_q), dtype=torch.float32, device="cuda")
     maps = torch.empty((len(kinds), grid.n_q), dtype=torch.float32, device="cuda")
-    nms.nms_amplitudes(ctx, grid, amp)
-    nms.nms_response(ctx, kinds, maps)
-    nms.nms_synchronize(ctx)
-    if n0 > 1:
-        assert nms.nms_get_info(ctx, "variant_used") == (3 if gtype == 0 else 5)
     qy, qz, th = oracle_mod.grid_points(grid)
     A, wsum = oracle_mod.amplitudes(pos, N, m, R, qy, qz, return_wsum=True)
     M = oracle_mod.response(A, th, kinds)
-    assert_amplitudes(amp.cpu().numpy(), A, wsum, f"ragged n0={n0}")
     misses = []
-    assert_cross_sections(maps.cpu().numpy(), M, kinds, f"ragged n0={n0}", signed_misses=misses)
+    for prec in (1, 0):                                     # fast (three-term, MUFU), then automatic = accurate
+        nms.nms_set_option(ctx, "precision", prec)
+        nms.nms_amplitudes(ctx, grid, amp)
+        nms.nms_response(ctx, kinds, maps)
+        nms.nms_synchronize(ctx)
+        if n0 > 1:
+            assert nms.nms_get_info(ctx, "variant_used") == (3 if gtype == 0 else 5)
+        assert (nms.nms_get_info(ctx, "poly_phasors") != 0) == (prec == 0)
+        assert_amplitudes(amp.cpu().numpy(), A, wsum, f"ragged n0={n0} precision {prec}")
+        assert_cross_sections(maps.cpu().numpy(), M, kinds, f"ragged n0={n0} precision {prec}", signed_misses=misses)
     report_signed_misses(misses)
 
 
@@ -278,15 +282,15 @@ def test_full_size_sampled(nms, ctx, oracle_mod, name, n_sample):
     nq = wl.grid.n_q
     amp = torch.empty((8, nq), dtype=torch.float32, device="cuda")
     maps = torch.empty((len(kinds), nq), dtype=torch.float32, device="cuda")
-    misses = []
     for R in rots:
         nms.nms_set_rotation(ctx, R)
         nms.nms_amplitudes(ctx, wl.grid, amp)
         nms.nms_response(ctx, kinds, maps)
         nms.nms_synchronize(ctx)
-        # an fp32-accumulating kernel: direct for C3 (log-spaced |q|), three-term line recurrence for C4 and C5
+        # an fp32-accumulating kernel: direct for C3 (log-spaced |q|), line recurrence for C4 and C5 -- the accurate
+        # variant, automatically: the amplitudes are kept for whatever kinds nms_response is asked for
         assert nms.nms_get_info(ctx, "variant_used") == {"C3": 2, "C4": 5, "C5": 3}[name]
-        assert nms.nms_get_info(ctx, "poly_phasors") == 0
+        assert nms.nms_get_info(ctx, "poly_phasors") != 0
         A_gpu, M_gpu = amp.cpu().numpy(), maps.cpu().numpy()
         A, wsum = oracle_mod.amplitudes(wl.pos, wl.N, wl.m, R, qy[idx], qz[idx], offsets=wl.offsets,
                                         centres=wl.centres, return_wsum=True)
@@ -297,9 +301,7 @@ def test_full_size_sampled(nms, ctx, oracle_mod, name, n_sample):
         # parents' maxima over the full GPU map as well
         pmax = {KI["NM"]: full_max[kinds.index(KI["NUC"])] + full_max[kinds.index(KI["PROJ"])],
                 KI["CHI"]: full_max[kinds.index(KI["SF"])]}
-        assert_cross_sections(M_gpu[:, idx], M, kinds, name, ref_max=full_max, parents=par, parent_max=pmax,
-                              signed_misses=misses)
-    report_signed_misses(misses)
+        assert_cross_sections(M_gpu[:, idx], M, kinds, name, ref_max=full_max, parents=par, parent_max=pmax)
 
 
 @pytest.fixture(scope="module")
@@ -311,15 +313,15 @@ def c5_full(oracle_mod):
     return wl, A, wsum, th
 
 
-@pytest.mark.parametrize("precision", [0, 2])
+@pytest.mark.parametrize("precision", [0, 1])
 def test_c5_full_map_end_to_end(nms, ctx, oracle_mod, c5_full, precision):
     """C5 at full size through the call sequence bench.py times (nms_compute, ring average, c(r), p(r)) against the
     FULL fp64 map of the oracle: all 13 maps at every one of the 262 144 detector points, the amplitudes, the 512-ring
     I(q) (Eq. 30) and c(r), p(r) at 1024 r (Eq. 34-35).
-    precision 0: the default kernel (three-term line recurrence, MUFU phasors) -- the configuration of the headline bench
-    line; a miss of NM / CHI is reported as xfail.  precision 2: the accurate variant (polynomial
-    phasors, rotations, fp64 sub-accumulation of the nuclear channel) -- every kind, NM and CHI included, must meet the
-    north_star criterion at every point."""
+    precision 0: what the library picks itself for C5's 13 kinds -- the accurate variant (polynomial phasors, rotations,
+    fp64 sub-accumulation of the nuclear channel), the configuration of the headline bench line: every kind, NM and CHI
+    included, must meet the north_star criterion at every point.  precision 1: the fast variant (three-term recurrence,
+    MUFU phasors) forced: a miss of NM / CHI is reported as xfail."""
     import torch
     wl, A, wsum, th = c5_full
     kinds = wl.kinds
@@ -338,10 +340,10 @@ def test_c5_full_map_end_to_end(nms, ctx, oracle_mod, c5_full, precision):
     nms.nms_amplitudes(ctx, wl.grid, amp)
     nms.nms_synchronize(ctx)
     assert nms.nms_get_info(ctx, "variant_used") == 3
-    assert (nms.nms_get_info(ctx, "poly_phasors") != 0) == (precision == 2)
+    assert (nms.nms_get_info(ctx, "poly_phasors") != 0) == (precision == 0)
     np.testing.assert_allclose(nms.nms_get_weight_sums(ctx), wsum, rtol=1e-12)
     assert_amplitudes(amp.cpu().numpy(), A, wsum, "C5 full map")
-    misses = [] if precision == 0 else None
+    misses = [] if precision == 1 else None
     assert_cross_sections(maps.cpu().numpy(), M, kinds, "C5 full map", signed_misses=misses)
     # 1-D outputs.  north_star states a criterion for the 2-D cross sections only; what it implies for a ring mean and
     # for its Fourier-Bessel transform follows by the triangle inequality: maps within 1e-3
@@ -418,7 +420,7 @@ def test_form_factor_split_small(nms, ctx, oracle_mod):
         tot_ref, form_ref = oracle_mod.form_factor_split(wl.pos, wl.N, wl.m, wl.offsets, kinds, qy, qz, th, R=wl.R,
                                                          centres=wl.centres, P=wl.P)
         misses = []
-        for variant, prec in ((0, 0), (1, 0), (1, 2)):   # exact kernel (automatic at this size), fp32 direct kernel, MUFU / polynomial
+        for variant, prec in ((0, 0), (1, 1), (1, 2)):   # exact kernel (automatic at this size), fp32 direct kernel, MUFU / polynomial
             nms.nms_set_option(ctx, "variant", variant)
             nms.nms_set_option(ctx, "precision", prec)
             for chunks in (0, 1, 3):
@@ -864,7 +866,7 @@ def test_ragged_cell_counts(nms, ctx, oracle_mod, W):
     amp = torch.empty((8, grid.n_q), dtype=torch.float32, device="cuda")
     # partial tiles of 1 ... 9 cells and tails behind full tiles through the bulk-copy / mbarrier kernels: direct with
     # 4 and 8 points per thread, MUFU and polynomial phasors, the line recurrence, and the exact kernel
-    for variant, qt, prec, used in ((1, 4, 0, 2), (1, 8, 0, 2), (1, 8, 2, 2), (2, 0, 0, 3), (2, 0, 2, 3), (0, 0, 0, 8)):
+    for variant, qt, prec, used in ((1, 4, 1, 2), (1, 8, 1, 2), (1, 8, 2, 2), (2, 0, 1, 3), (2, 0, 0, 3), (0, 0, 0, 8)):
         nms.nms_set_option(ctx, "variant", variant)
         nms.nms_set_option(ctx, "qt", qt)
         nms.nms_set_option(ctx, "precision", prec)
@@ -876,7 +878,7 @@ def test_ragged_cell_counts(nms, ctx, oracle_mod, W):
         assert_amplitudes(amp.cpu().numpy(), A, wsum, f"W={W} variant={variant} qt={qt} precision={prec}")
 
 
-@pytest.mark.parametrize("variant,prec", [(0, 0), (1, 0), (1, 2)])
+@pytest.mark.parametrize("variant,prec", [(0, 0), (1, 1), (1, 0)])
 def test_list_grid_against_oracle(nms, ctx, oracle_mod, variant, prec):
     """A point-list detector with random non-zero q (MODE 2 kernel, 4 points per thread): amplitudes and all kinds."""
     import torch
@@ -929,9 +931,10 @@ def test_recurrence_far_from_the_origin(nms, ctx, oracle_mod, gtype):
     M = oracle_mod.response(A, th, kinds)
     amp = torch.empty((8, grid.n_q), dtype=torch.float32, device="cuda")
     maps = torch.empty((len(kinds), grid.n_q), dtype=torch.float32, device="cuda")
-    for rec in (1, 2):
+    for rec, prec in ((1, 1), (2, 1), (0, 2)):
         nms.nms_set_option(ctx, "variant", 2)
         nms.nms_set_option(ctx, "recurrence", rec)
+        nms.nms_set_option(ctx, "precision", prec)
         nms.nms_amplitudes(ctx, grid, amp)
         nms.nms_response(ctx, kinds, maps)
         nms.nms_synchronize(ctx)
@@ -1093,21 +1096,25 @@ def test_batched_fields(nms, ctx, oracle_mod, gtype):
     nq = grid.n_q
     maps = torch.empty((B, len(kinds), nq), dtype=torch.float32, device="cuda")
     amp = torch.empty((B, 8, nq), dtype=torch.float32, device="cuda")
-    nms.nms_compute_batch(ctx, grid, _t(mb), kinds, maps, amp)
-    nms.nms_synchronize(ctx)
     qy, qz, th = oracle_mod.grid_points(grid)
     A = oracle_mod.amplitudes_batch(wl.pos, wl.N, mb, R, qy, qz)
-    a_h, m_h = amp.cpu().numpy(), maps.cpu().numpy()
     misses = []
-    for b in range(B):
-        _, wsum = oracle_mod.amplitudes(wl.pos, wl.N, mb[b], R, qy[:1], qz[:1], return_wsum=True)
-        assert_amplitudes(a_h[b], A[b], wsum, f"field {b}")
-        assert np.array_equal(a_h[b, 0:2], a_h[0, 0:2])                              # one nuclear amplitude for all fields
-        M = oracle_mod.response(A[b], th, kinds)
-        assert_cross_sections(m_h[b], M, kinds, f"field {b}", signed_misses=misses)
+    for prec in (1, 0):                                     # fast (MUFU), then automatic = accurate (signed kinds asked for)
+        nms.nms_set_option(ctx, "precision", prec)
+        nms.nms_compute_batch(ctx, grid, _t(mb), kinds, maps, amp)
+        nms.nms_synchronize(ctx)
+        assert (nms.nms_get_info(ctx, "poly_phasors") != 0) == (prec == 0)
+        a_h, m_h = amp.cpu().numpy(), maps.cpu().numpy()
+        for b in range(B):
+            _, wsum = oracle_mod.amplitudes(wl.pos, wl.N, mb[b], R, qy[:1], qz[:1], return_wsum=True)
+            assert_amplitudes(a_h[b], A[b], wsum, f"field {b}")
+            assert np.array_equal(a_h[b, 0:2], a_h[0, 0:2])                          # one nuclear amplitude for all fields
+            M = oracle_mod.response(A[b], th, kinds)
+            assert_cross_sections(m_h[b], M, kinds, f"field {b} precision {prec}", signed_misses=misses)
     # the ordinary path on field 3 gives the same maps within the criterion
     nms.nms_set_sample(ctx, _t(wl.pos), _t(wl.N), _t(mb[3]), R)
     nms.nms_set_option(ctx, "variant", 1)
+    nms.nms_set_option(ctx, "precision", 0)
     one = torch.empty((len(kinds), nq), dtype=torch.float32, device="cuda")
     nms.nms_compute(ctx, grid, kinds, one)
     nms.nms_synchronize(ctx)
@@ -1146,6 +1153,7 @@ def test_friedel_halving(nms, ctx, oracle_mod, name, small, variant):
     _upload(nms, ctx, wl)
     nms.nms_set_option(ctx, "variant", variant)
     nms.nms_set_option(ctx, "friedel", 1)
+    nms.nms_set_option(ctx, "precision", 1)    # nms_amplitudes and nms_compute (positive kinds) would otherwise differ in variant
     nq = wl.grid.n_q
     amp = torch.empty((8, nq), dtype=torch.float32, device="cuda")
     maps = torch.empty((len(kinds), nq), dtype=torch.float32, device="cuda")
