@@ -21,7 +21,9 @@
 //                   minimax sin (degree 7) and cos (degree 8) on [-pi/4, pi/4] (approximation errors 1.8e-9, 1e-10),
 //                   quadrant swap and signs from the top two bits.  Emulated in fp32: max error 8.3e-8, rms 1.8e-8 per
 //                   component, every Fourier component of the error function below 5e-10.
-//                   19 issue slots, none on the XU pipe.
+//                   19 issue slots, none on the XU pipe.  (Evaluating the same polynomials in fp64 on the FP64 pipe,
+//                   idle at 6 % in the accurate recurrence kernel, was measured SLOWER: C5 0.567 -> 0.525 with the step
+//                   phasor alone in fp64, 0.483 with both; mixing three-term steps into the rotations gained nothing.)
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
