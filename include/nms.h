@@ -159,7 +159,7 @@ NMS_API nms_status nms_compute(nms_ctx* ctx, const nms_qgrid* grid, const nms_ki
  * The phasors and the nuclear sum are evaluated once per group of 3 fields and shared; field b gets the same results as
  * nms_set_sample(pos, N, m_batch[b]) + nms_compute would give.  out_maps [dev][n_fields][n_kinds][n_q] (float) or NULL;
  * out_amp [dev][n_fields][8][n_q] (float, plane order as nms_amplitudes; planes 0-1 are the shared nuclear amplitude) or
- * NULL (not both NULL).  fp32 kernels with MUFU phasors (as the direct kernel of nms_compute) at every problem size.  */
+ * NULL (not both NULL).  fp32 kernels at every problem size, fast or accurate variant by the "precision" rule below.  */
 NMS_API nms_status nms_compute_batch(nms_ctx* ctx, const nms_qgrid* grid, const float* m_batch, int n_fields,
                              const nms_kind* kinds, int n_kinds, float* out_maps, float* out_amp);
 
@@ -256,10 +256,16 @@ NMS_API nms_status nms_get_weight_sums(nms_ctx* ctx, double* out);
  * kernel where u0 is equally spaced and the cell order is spatially coherent, else the direct kernel), 1 force the
  * direct (one phasor per pair) kernel, 2 force the line-recurrence kernel (NMS_E_UNSUPPORTED at compute time if the
  * detector is a point list or u0 is not an arithmetic progression within one fp32 ulp), 3 force the exact fp64
- * kernel.  "precision": 0 / 1 MUFU phasors (sin.approx / cos.approx on the exactly reduced phase), 2 polynomial
- * phasors on the FMA pipe, accurate to fp32 rounding (the selectable accurate variant of the fp32 kernels: 25-50 %
- * slower).  "bases": exactly evaluated points per 8 in the recurrence kernel (0 auto = 1, else
- * 1..4).  "recurrence": 0 auto, 1 complex rotations, 2 three-term recurrence (bases <= 2).  "timing": 1 records a
+ * kernel.  "precision": which variant of the fp32 kernels runs.  1 fast: MUFU phasors (sin.approx /
+ * cos.approx on the exactly reduced phase), three-term recurrence; amplitudes and the positive kinds meet the north-star
+ * tolerances, the signed difference kinds NM and CHI miss them at a fraction of a percent of their points.  2 accurate:
+ * polynomial phasors to fp32 rounding, rotations, fp64 sub-accumulation of the nuclear channel; 25-30 % slower; meets the
+ * tolerances for all 13 kinds on every config.  0 (default) automatic: accurate where NM / CHI may be formed from the sums
+ * (nms_amplitudes, whose result nms_response and nms_cross_spectra use later; nms_compute, nms_form_factor_split and
+ * nms_compute_batch when NMS_NM or NMS_CHI is among the kinds or amplitudes are returned), fast otherwise.
+ * "bases": exactly evaluated points per 8 in the recurrence kernel (0 auto = 1, else
+ * 1..4).  "recurrence": 0 auto (three-term in the fast variant, rotations in the accurate one), 1 complex rotations, 2 three-term
+ * recurrence (bases <= 2).  "timing": 1 records a
  * CUDA event pair around every kernel launch (and resets the record).  "chunks": 0 auto, else the number of cell
  * chunks.  "qt": 0 auto, else detector points per thread (4 or 8; 16 for the recurrence kernel on a sample without
  * moments).  "friedel" (f-4): 1 = on a polar grid with an even number of angles closed under theta -> theta + pi
