@@ -659,7 +659,8 @@ def run_cuda(args, rank, local_rank, world):
 
     wl_full = ni.make_config(args.workload)
     sharded = world > 1 and (args.shard == "lines" or (args.shard == "auto" and can_shard_lines(wl_full, world)))
-    res = measure(nms, torch, wl_full, args, args.steps, args.warmup, dist, rank, local_rank, world, sharded, True)
+    res = measure(nms, torch, wl_full, args, args.steps, args.warmup, dist, rank, local_rank, world, sharded, True,
+                  precision=args.precision)
     # the other two throughput configs of the north-star target (>= 60 % on C3-C5), timed OUTSIDE the headline region
     configs = None
     if world == 1 and not args.no_configs:
@@ -693,7 +694,7 @@ def run_cuda(args, rank, local_rank, world):
                 "warmup": args.warmup, "ms_per_step": res["ms_per_step"], "higher_is_better": True,
                 "scaling": "strong" if sharded else "weak",
                 "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-                "config": workload_config(wl_full, {"parallelism": ("detector lines sharded over ranks, cells replicated, all-gather of I(q) only"
+                "config": workload_config(wl_full, {"precision_option": args.precision, "parallelism": ("detector lines sharded over ranks, cells replicated, all-gather of I(q) only"
                                                                     if sharded else "replicas only") if world > 1 else "single GPU"}),
                 "clocks": res["clocks"], "e2e": res["e2e"], "gpu_launches": res["gpu_launches"], "roofline": res["roofline"],
                 "passes": res["passes"], "next_rows": res["next_rows"], "cpu_baseline": res["cpu_baseline"],
@@ -720,6 +721,8 @@ def main():
     ap.add_argument("--pipes", action="store_true",
                     help="measured issue rates of the instruction classes of the amplitude kernels and error statistics "
                          "of the two phasor routines (one JSON line; the table behind DESIGN.md section 6)")
+    ap.add_argument("--precision", type=int, default=0, choices=[0, 1, 2],
+                    help="kernel variant of the timed workload: 0 the library's own choice (default), 1 fast, 2 accurate")
     ap.add_argument("--no-configs", action="store_true", help="skip the C3 / C4 side measurements of the default line")
     args = ap.parse_args()
     rank, local_rank, world = _env_int("RANK", 0), _env_int("LOCAL_RANK", 0), _env_int("WORLD_SIZE", 1)
