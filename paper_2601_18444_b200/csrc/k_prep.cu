@@ -35,6 +35,16 @@ __device__ __forceinline__ double warp_sum(double v)
     return v;
 }
 
+// Bounding box and radius need no more than float accuracy (tile centres for a first-order correction, a range check):
+// order-preserving integer images of the floats go through the warp-wide REDUX instruction (1 instead of 10 shuffles).
+__device__ __forceinline__ int float_order(float f)
+{
+    const int i = __float_as_int(f);
+    return i >= 0 ? i : i ^ 0x7fffffff;
+}
+__device__ __forceinline__ float order_float(int i) { return __int_as_float(i >= 0 ? i : i ^ 0x7fffffff); }
+__device__ __forceinline__ float warp_minf(float v) { return order_float(__reduce_min_sync(0xffffffffu, float_order(v))); }
+__device__ __forceinline__ float warp_maxf(float v) { return order_float(__reduce_max_sync(0xffffffffu, float_order(v))); }
 __device__ __forceinline__ double warp_min(double v)
 {
     for (int o = 16; o > 0; o >>= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, o));
@@ -91,7 +101,9 @@ __global__ void __launch_bounds__(PREP_THREADS) k_prep(const PrepArgs a)
         }
     }
     sN = warp_sum(sN); sx = warp_sum(sx); sy = warp_sum(sy); sz = warp_sum(sz);
-    ylo = warp_min(ylo); yhi = warp_max(yhi); zlo = warp_min(zlo); zhi = warp_max(zhi); r2 = warp_max(r2);
+    // rounded outwards by one float ulp at most: harmless for a centre, conservative for the radius
+    ylo = (double)warp_minf((float)ylo); yhi = (double)warp_maxf((float)yhi);
+    zlo = (double)warp_minf((float)zlo); zhi = (double)warp_maxf((float)zhi); r2 = (double)warp_maxf((float)r2 * 1.0000002f);
     if (lane == 0) {
         red[0][warp] = sN; red[1][warp] = sx; red[2][warp] = sy; red[3][warp] = sz;
         red[4][warp] = ylo; red[5][warp] = yhi; red[6][warp] = zlo; red[7][warp] = zhi; red[8][warp] = r2;
