@@ -20,6 +20,16 @@ amp_kernel_t amp_kernel_rec_cart(int qt, int nb, bool split, int nch, bool poly,
         if (rec3) return split ? (amp_kernel_t)k_amp<1, 8, true, 4, 1, 4, 1, 1, false, true> : (amp_kernel_t)k_amp<1, 8, false, 4, 1, 4, 1, 1, false, true>;
         return split ? (amp_kernel_t)k_amp<1, 8, true, 4, 1, 4, 1, 0, false, true> : (amp_kernel_t)k_amp<1, 8, false, 4, 1, 4, 1, 0, false, true>;
     }
+    // 16 points per thread at 2 blocks per SM (four channels, not split): the fast variant with 2 exact points and the
+    // three-term recurrence (the arithmetic of 8 points with 1), the accurate variant with 1 exact point and rotations
+    if (qt == 16) {
+        if (nch == 4 && !split) {
+            if (!poly && rec3 && nb == 2) return (amp_kernel_t)k_amp<1, 16, false, 2, 2, 4, 0, 1>;
+            if (poly && !rec3 && nb == 1)
+                return sh ? (amp_kernel_t)k_amp<1, 16, false, 2, 1, 4, 1, 0, false, true> : (amp_kernel_t)k_amp<1, 16, false, 2, 1, 4, 1, 0>;
+            return nullptr;
+        }
+    }
     (void)uni;   // no gain measured on Cartesian lines (C4: 0.8136 against 0.8120)
     if (nch == 1) {
         if (split) return nullptr;

@@ -20,6 +20,16 @@ amp_kernel_t amp_kernel_rec_polar(int qt, int nb, bool split, int nch, bool poly
         if (rec3) return split ? (amp_kernel_t)k_amp<0, 8, true, 4, 1, 4, 1, 1, false, true> : (amp_kernel_t)k_amp<0, 8, false, 4, 1, 4, 1, 1, false, true>;
         return split ? (amp_kernel_t)k_amp<0, 8, true, 4, 1, 4, 1, 0, false, true> : (amp_kernel_t)k_amp<0, 8, false, 4, 1, 4, 1, 0, false, true>;
     }
+    // 16 points per thread at 2 blocks per SM (four channels, not split): the fast variant with 2 exact points and the
+    // three-term recurrence (the arithmetic of 8 points with 1), the accurate variant with 1 exact point and rotations
+    if (qt == 16) {
+        if (nch == 4 && !split) {
+            if (!poly && rec3 && nb == 2) return (amp_kernel_t)k_amp<0, 16, false, 2, 2, 4, 0, 1>;
+            if (poly && !rec3 && nb == 1)
+                return sh ? (amp_kernel_t)k_amp<0, 16, false, 2, 1, 4, 1, 0, false, true> : (amp_kernel_t)k_amp<0, 16, false, 2, 1, 4, 1, 0>;
+            return nullptr;
+        }
+    }
     // the default fast kernel with block-uniform line abscissae (n1 a multiple of 128): C5 0.783 -> 0.804 of the roofline
     if (uni && qt == 8 && nb == 1 && nch == 4 && !poly && rec3)
         return split ? (amp_kernel_t)k_amp<0, 8, true, 4, 1, 4, 0, 1, true> : (amp_kernel_t)k_amp<0, 8, false, 4, 1, 4, 0, 1, true>;

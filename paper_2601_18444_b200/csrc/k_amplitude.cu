@@ -151,7 +151,11 @@ nms_status plan_amplitude(nms_ctx* c, bool split, bool want_accurate, AmpPlan* p
     int qt_opts[3]; int n_opts = 0;
     if (p.variant == 8) { qt_opts[n_opts++] = 1; }
     else if (p.variant == 1) { qt_opts[n_opts++] = 4; }
-    else if (rec) { if (p.nch == 1 && c->opt_bases == 0) qt_opts[n_opts++] = 16; qt_opts[n_opts++] = 8; }
+    else if (rec) {   // 16 points per thread: one channel, or four channels (2 blocks per SM) in the default arrangements
+        const bool defaults = c->opt_bases == 0 && c->opt_rec3 == 0;
+        if (defaults && (p.nch == 1 || !split)) qt_opts[n_opts++] = 16;
+        qt_opts[n_opts++] = 8;
+    }
     else { qt_opts[n_opts++] = 8; qt_opts[n_opts++] = 4; }
     p.qt = qt_opts[n_opts - 1];
     if (c->opt_qt && p.variant != 8) {
@@ -168,7 +172,7 @@ nms_status plan_amplitude(nms_ctx* c, bool split, bool want_accurate, AmpPlan* p
     // recurrence: one exactly evaluated point per 8 and the three-term recurrence (measured fastest: C5 0.69 -> 0.785 of
     // the roofline against 2 bases + rotations, errors of the same size); the accurate variant keeps the rotations
     if (rec) {
-        p.nb = c->opt_bases ? c->opt_bases : (p.qt == 16 ? 4 : (p.nch == 1 ? 2 : 1));
+        p.nb = c->opt_bases ? c->opt_bases : (p.nch == 1 ? (p.qt == 16 ? 4 : 2) : (p.qt == 16 && !accurate ? 2 : 1));
         p.rec3 = c->opt_rec3 ? (c->opt_rec3 == 2) : (!accurate && (p.qt == 16 || p.nb <= 2));
         p.npoly = accurate ? 1 : 0;
         if (p.rec3 && p.qt == 8 && p.nb > 2) return fail(c, NMS_E_ARG, "the three-term recurrence needs bases <= 2");

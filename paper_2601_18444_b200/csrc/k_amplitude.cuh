@@ -197,6 +197,8 @@ template <int QT, int NB> struct Seg {
 //         REC3 = 1: three-term recurrence instead of rotations.
 // UNI: the launch guarantees n1 % 128 == 0, so a block lies inside ONE group of QT lines: the line abscissae are then
 //      block-uniform values (derived from blockIdx only), which frees the 2 QT registers a thread needs for them.
+// QT = 16 with four channels: 128 accumulator registers, built with MINB = 2 (255 registers, 8 warps per SM); measured on C5
+//      against QT = 8 at 128 registers and 16 warps per SM: fast variant 0.805 -> 0.857 of the roofline, accurate 0.566 -> 0.634.
 // SH:  polynomial recurrence kernels only: the step phase stays within a quarter cycle (checked on the host: d r_max <
 //      pi / 2), so the step phasor needs no quadrant logic (sincos_poly_half).
 template <int MODE, int QT, bool SPLIT, int MINB, int NB, int NCH, int NPOLY, int REC3, bool UNI = false, bool SH = false>
@@ -334,6 +336,16 @@ __global__ void __launch_bounds__(AMP_THREADS, MINB) k_amp(const AmpArgs a)
                         for (int k = kb + 2; k <= S::hi(b); ++k) ph[k] = three_term(ph[k - 1], ph[k - 2], two_cd);
 #pragma unroll
                         for (int k = kb - 1; k >= S::lo(b); --k) ph[k] = three_term(ph[k + 1], ph[k + 2], two_cd);
+                    } else if (QT / NBX >= 16) {
+                        // long segments: two interleaved chains per direction, advanced by the squared step phasor
+                        // (half the depth of the dependency chain and of the accumulated rotation roundings)
+                        const float c2 = fmaf(-2.f * sd, sd, 1.f), s2 = 2.f * sd * cd;
+                        if (S::hi(b) > kb) ph[kb + 1] = rotate(ph[kb], cd, sd);
+                        if (S::lo(b) < kb) ph[kb - 1] = rotate(ph[kb], cd, -sd);
+#pragma unroll
+                        for (int k = kb + 2; k <= S::hi(b); ++k) ph[k] = rotate(ph[k - 2], c2, s2);
+#pragma unroll
+                        for (int k = kb - 2; k >= S::lo(b); --k) ph[k] = rotate(ph[k + 2], c2, -s2);
                     } else {
 #pragma unroll
                         for (int k = kb + 1; k <= S::hi(b); ++k) ph[k] = rotate(ph[k - 1], cd, sd);
