@@ -150,11 +150,13 @@ def _run_full(nms, h, wl, kinds):
 @pytest.mark.parametrize("variant,qt,bases,rec,prec", [(0, 0, 0, 0, 0), (3, 0, 0, 0, 0), (1, 0, 0, 0, 1), (1, 4, 0, 0, 1),
                                                         (1, 8, 0, 0, 1), (1, 0, 0, 0, 2), (1, 4, 0, 0, 0),
                                                         (2, 0, 0, 0, 1), (2, 0, 1, 1, 1), (2, 0, 2, 1, 1), (2, 0, 2, 2, 1),
-                                                        (2, 0, 3, 1, 1), (2, 0, 4, 1, 1), (2, 0, 0, 0, 0), (2, 0, 2, 2, 2)])
+                                                        (2, 0, 3, 1, 1), (2, 0, 4, 1, 1), (2, 0, 0, 0, 0), (2, 0, 2, 2, 2),
+                                                        (2, 16, 0, 0, 1), (2, 16, 0, 0, 0)])
 def test_full_config_maps(nms, ctx, oracle_mod, name, variant, qt, bases, rec, prec):
     """variant 0 = automatic (these small problems run the exact fp64 kernel), 3 = exact forced: every kind held to
     the north_star criterion.  1 = the fp32-accumulating direct kernels, 2 = the line-recurrence kernels with `bases`
-    exactly evaluated points per 8 by rotations (rec 1) or the three-term recurrence (rec 2), MUFU (prec 1) or
+    exactly evaluated points per 8 by rotations (rec 1) or the three-term recurrence (rec 2) -- qt 16: the 16-point
+    kernels large problems get, 2 exact points + three-term (fast) or 1 + rotations (accurate) --, MUFU (prec 1) or
     polynomial (prec 2; prec 0 = automatic, which is 2 here: all 13 kinds are asked for) phasors: amplitudes and every
     kind to the same criterion; a miss of NM / CHI is reported as xfail (C1 and C2 are below the size where the library
     itself would pick an fp32 kernel)."""
@@ -179,7 +181,8 @@ def test_full_config_maps(nms, ctx, oracle_mod, name, variant, qt, bases, rec, p
     if variant in (1, 2):
         assert (nms.nms_get_info(ctx, "poly_phasors") != 0) == (prec != 1)
     if variant == 2:
-        assert nms.nms_get_info(ctx, "bases") == (bases or 1)
+        assert nms.nms_get_info(ctx, "bases") == (bases or (2 if qt == 16 and prec == 1 else 1))
+        assert nms.nms_get_info(ctx, "qt") == (qt or 8)
         assert nms.nms_get_info(ctx, "three_term") == (1 if rec == 2 or (rec == 0 and prec == 1) else 0)
     report_signed_misses(misses)
 
@@ -227,10 +230,11 @@ def test_small_config_maps(nms, ctx, oracle_mod, name, variant, prec):
 
 
 @pytest.mark.parametrize("gtype", [0, 1])
-@pytest.mark.parametrize("n0", [1, 2, 7, 13, 24])
-def test_recurrence_ragged_lines(nms, ctx, oracle_mod, gtype, n0):
-    """Line recurrence on detector lines whose length is not a multiple of the 8 points a thread owns (and
-    shorter than them): the points beyond the edge continue the progression and are never stored."""
+@pytest.mark.parametrize("n0,qt", [(1, 0), (2, 0), (7, 0), (13, 0), (24, 0), (2, 16), (13, 16), (24, 16), (33, 16)])
+def test_recurrence_ragged_lines(nms, ctx, oracle_mod, gtype, n0, qt):
+    """Line recurrence on detector lines whose length is not a multiple of the 8 or 16 points a thread owns (and
+    shorter than them): the points beyond the edge continue the progression and are never stored.  qt = 16 forces the
+    16-point kernels that large problems get (this one is too small to be given them automatically)."""
     rng = np.random.Generator(np.random.Philox(4242))
     W = 3000
     pos = rng.uniform(-40, 40, size=(W, 3)).astype(np.float32)
@@ -245,6 +249,7 @@ def test_recurrence_ragged_lines(nms, ctx, oracle_mod, gtype, n0):
     import torch
     nms.nms_set_sample(ctx, _t(pos), _t(N), _t(m), R)
     nms.nms_set_option(ctx, "variant", 2 if n0 > 1 else 1)
+    nms.nms_set_option(ctx, "qt", qt)
     amp = torch.empty((8, grid.n_q), dtype=torch.float32, device="cuda")
     maps = torch.empty((len(kinds), grid.n_q), dtype=torch.float32, device="cuda")
     qy, qz, th = oracle_mod.grid_points(grid)
@@ -258,6 +263,7 @@ def test_recurrence_ragged_lines(nms, ctx, oracle_mod, gtype, n0):
         nms.nms_synchronize(ctx)
         if n0 > 1:
             assert nms.nms_get_info(ctx, "variant_used") == (3 if gtype == 0 else 5)
+            assert nms.nms_get_info(ctx, "qt") == (qt if qt else 8)
         assert (nms.nms_get_info(ctx, "poly_phasors") != 0) == (prec == 0)
         assert_amplitudes(amp.cpu().numpy(), A, wsum, f"ragged n0={n0} precision {prec}")
         assert_cross_sections(maps.cpu().numpy(), M, kinds, f"ragged n0={n0} precision {prec}", signed_misses=misses)
