@@ -175,6 +175,18 @@ NMS_API nms_status nms_compute_batch(nms_ctx* ctx, const nms_qgrid* grid, const 
  * [dev][n_bins] (int32) or NULL.                                                                 */
 NMS_API nms_status nms_azimuthal_average(nms_ctx* ctx, const float* maps, int n_maps, int n_bins, double q_lo,
                                  double q_hi, float* out_I, float* out_q, int32_t* out_count);
+/* The |q|-histogram mode of nms_azimuthal_average (q_hi > q_lo, any grid type; Eq. 30, reading 8) for callers that
+ * cannot allocate device memory (CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc): same
+ * arguments, same results (counts identical, averages equal up to the order of the fp64 additions), but the call
+ * allocates and frees nothing.  Its scratch -- per-bin counts and per-(map, bin) fp64 sums -- is one static device array
+ * of 576 KB inside libnms.so, held by every GPU that loads the library until the process exits.  Limits: n_bins <= 16384
+ * and n_maps * n_bins <= 65536 (NMS_E_UNSUPPORTED beyond them); q_hi <= q_lo (the ring mode, which uses no scratch) is
+ * NMS_E_ARG.  The first call on a device resolves the array's address (cudaGetSymbolAddress): make it outside any graph
+ * capture.  Every call on a device shares the array, and it keeps the last call's contents: each call clears what it uses
+ * on the context's stream first; calls that overlap on the GPU (two streams, two contexts) RACE -- serialise them.
+ * Asynchronous on the context's stream like the other calls.                                                          */
+NMS_API nms_status nms_azimuthal_average_noalloc(nms_ctx* ctx, const float* maps, int n_maps, int n_bins, double q_lo,
+                                         double q_hi, float* out_I, float* out_q, int32_t* out_count);
 
 /* ---- angular modal decomposition (f-2, Eq. 31-33) -------------------------------------- */
 

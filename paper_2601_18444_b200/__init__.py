@@ -35,6 +35,7 @@ EXPORTS = [
     "nms_azimuthal_average", "nms_correlation", "nms_form_factor_split", "nms_run_host", "nms_get_weight_sums",
     "nms_set_option", "nms_get_info", "nms_kernel_time_ms", "nms_kernel_time_total", "nms_modal_decomposition",
     "nms_correlation_2d", "nms_cross_spectra", "nms_run_host_split", "nms_run_host_scan", "nms_pipe_rates", "nms_phasor_selftest", "nms_compute_batch",
+    "nms_azimuthal_average_noalloc",
 ]
 
 
@@ -193,6 +194,13 @@ def nms_form_factor_split(ctx, grid, kinds, out_total, out_form):
 def nms_azimuthal_average(ctx, maps, n_maps, n_bins, q_lo, q_hi, out_I, out_q=None, out_count=None):
     _check(ctx, _lib.nms_azimuthal_average(ctx, _dev(maps), C.c_int(n_maps), C.c_int(n_bins), C.c_double(q_lo),
                                            C.c_double(q_hi), _dev(out_I), _dev(out_q), _dev(out_count)))
+
+
+def nms_azimuthal_average_noalloc(ctx, maps, n_maps, n_bins, q_lo, q_hi, out_I, out_q=None, out_count=None):
+    """|q|-histogram average that allocates nothing (static 576 KB scratch in libnms.so; n_bins <= 16384, n_maps * n_bins
+    <= 65536; calls that overlap on the GPU race on the scratch)."""
+    _check(ctx, _lib.nms_azimuthal_average_noalloc(ctx, _dev(maps), C.c_int(n_maps), C.c_int(n_bins), C.c_double(q_lo),
+                                                   C.c_double(q_hi), _dev(out_I), _dev(out_q), _dev(out_count)))
 
 
 def nms_modal_decomposition(ctx, maps, n_maps, k_max, out_Is=None, out_Ic=None, out_a=None, out_A=None):
