@@ -159,7 +159,10 @@ NMS_API nms_status nms_compute(nms_ctx* ctx, const nms_qgrid* grid, const nms_ki
  * The phasors and the nuclear sum are evaluated once per group of 3 fields and shared; field b gets the same results as
  * nms_set_sample(pos, N, m_batch[b]) + nms_compute would give.  out_maps [dev][n_fields][n_kinds][n_q] (float) or NULL;
  * out_amp [dev][n_fields][8][n_q] (float, plane order as nms_amplitudes; planes 0-1 are the shared nuclear amplitude) or
- * NULL (not both NULL).  fp32 kernels at every problem size, fast or accurate variant by the "precision" rule below.  */
+ * NULL (not both NULL).  fp32 kernels at every problem size, fast or accurate variant by the "precision" rule below;
+ * the accurate variant runs a line recurrence over 8 points per thread where u0 is equally spaced and the cell order
+ * spatially coherent; otherwise (fast variant, list detectors, "variant" 1) the direct kernel with 4 points per thread;
+ * "variant" 2 forces the recurrence (NMS_E_UNSUPPORTED without equally spaced lines).                                 */
 NMS_API nms_status nms_compute_batch(nms_ctx* ctx, const nms_qgrid* grid, const float* m_batch, int n_fields,
                              const nms_kind* kinds, int n_kinds, float* out_maps, float* out_amp);
 
@@ -290,7 +293,8 @@ NMS_API nms_status nms_get_weight_sums(nms_ctx* ctx, double* out);
  * otherwise; the exact kernel has no such limit).                                                        */
 NMS_API nms_status nms_set_option(nms_ctx* ctx, const char* key, int64_t value);
 /* Read back integers: "launches" (kernels launched by this context so far), "variant_used" (1 list direct,
- * 2 polar direct, 4 cartesian direct, 3 polar recurrence, 5 cartesian recurrence, 8 exact fp64),
+ * 2 polar direct, 4 cartesian direct, 3 polar recurrence, 5 cartesian recurrence, 8 exact fp64, 16 / 17 batched-field
+ * kernel direct / line recurrence),
  * "n_chunks", "n_tiles", "n_slots", "sm_count", "blocks_per_sm", "qt", "poly_phasors" (non-zero: polynomial phasors),
  * "bases", "three_term", "corr2d_variant" (variant_used of the last nms_correlation_2d).             */
 NMS_API nms_status nms_get_info(nms_ctx* ctx, const char* key, int64_t* value);

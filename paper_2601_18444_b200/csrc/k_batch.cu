@@ -7,15 +7,19 @@
 // m'z)} (k_prep_batch: rotation in fp64, one rounding, as a-1), and k_amp_batch evaluates ONE phasor per (cell, detector
 // point) and feeds it to 10 packed accumulations (1 nuclear + 9 magnetic) instead of 4: 20 FMA-pipe cycles + ~6 issue slots
 // for the phasor per 3 pair-fields against 3 x (8 + ~6) -- 8.7 instead of 14 cycles per pair-field.  With 10 complex
-// accumulators per point a thread owns QT = 4 points (80 registers); the 2 MUFU per pair then need 16 XU cycles against 20
-// FMA cycles, so the direct evaluation is no longer XU-bound and no recurrence is needed (any detector grid).
+// accumulators per point a thread owns QT = 4 points (80 registers, 3 blocks per SM) in the DIRECT kernel (any detector
+// grid: the 2 MUFU per pair need 16 XU cycles against 20 FMA cycles, so it is not XU-bound), and QT = 8 points (160
+// registers, 2 blocks per SM) in the LINE-RECURRENCE kernel that the accurate variant runs on equally spaced lines: one
+// exactly evaluated point per 8, the others by rotations (accurate) or rotation + three-term recurrence (fast, on request
+// only), as in k_amplitude.cuh.
 // k_epilogue_batch sums the chunk partials and forms the requested responses of every field of the group with the shared N~.
 #include "k_amplitude.cuh"
 
 namespace nms {
 
 constexpr int BF = 3;              // fields per pass
-constexpr int BQT = 4;             // detector points per thread
+constexpr int BQT = 4;             // detector points per thread, direct kernel
+constexpr int BQT_REC = 8;         // detector points per thread, line-recurrence kernel
 constexpr int BCH = 1 + 3 * BF;    // weight channels per record
 
 struct BCell {                     // 64 B
@@ -30,6 +34,8 @@ struct BatchArgs {
     int type, n0, n1;
     int64_t n_q;
     const float* u0;
+    double dq;                     // recurrence: spacing of u0
+    int sh;                        // recurrence, accurate: the step phase stays within a quarter cycle
     const double2* qc;
     const double2* sc;
     double* part;                  // [n_chunks][2 * BCH][n_q]
@@ -88,9 +94,15 @@ constexpr size_t BATCH_SMEM = 2 * TILE * sizeof(BCell) + 2 * sizeof(uint64_t);
 // 3 blocks per SM: 80 accumulator registers + phase constants need ~150 registers (at 128 the kernel spills and was
 // measured 20 % slower: C5 2578 against 3084 Gpair-field/s).
 // ACC: the accurate variant (polynomial phasor, fp64 sub-accumulation of the shared nuclear channel every NSUB_CELLS cells).
-template <int MODE, bool ACC>
-__global__ void __launch_bounds__(AMP_THREADS, 3) k_amp_batch(const BatchArgs a)
+// REC: line recurrence over the thread's BQT = 8 points (MODE 0 / 1 with equally spaced u0; 2 blocks per SM): the point
+//      KB is evaluated exactly, fast variant: its upper neighbour by one rotation and the others by the three-term
+//      recurrence (runs of <= 3 steps); accurate variant: rotations both ways (<= 4 steps).  The deviation of the float
+//      abscissae from the progression is corrected at the flush, to first order, at the tile centre (as k_amp).
+template <int MODE, bool ACC, int BQT, bool REC>
+__global__ void __launch_bounds__(AMP_THREADS, REC ? 2 : 3) k_amp_batch(const BatchArgs a)
 {
+    static_assert(!REC || MODE != 2, "the recurrence needs a line of equally spaced abscissae");
+    constexpr int KB = ACC ? BQT / 2 : (BQT - 1) / 2;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     BCell* sC = reinterpret_cast<BCell*>(smem_raw);
     uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + 2 * TILE * sizeof(BCell));
@@ -119,6 +131,9 @@ __global__ void __launch_bounds__(AMP_THREADS, 3) k_amp_batch(const BatchArgs a)
     }
     if (MODE == 0) { const double2 d = a.sc[flat0]; c0 = d.x; c1 = d.y; }
     if (MODE == 1) c0 = h[0];
+    const double dq = a.dq * INV_2PI;
+    double gb = g[KB < BQT ? KB : 0];   // abscissa of the exactly evaluated point; beyond the edge it continues the progression
+    if (REC && KB >= kclamp) gb += (double)(KB - (kclamp - 1)) * dq;
 
     auto issue = [&](int tile, BCell* dst, uint64_t* b) {
         const TileMeta tm = a.tiles[tile];
@@ -141,7 +156,8 @@ __global__ void __launch_bounds__(AMP_THREADS, 3) k_amp_batch(const BatchArgs a)
     u64 acc[BQT][BCH];
     for (int t = tile_beg; t < tile_end; ++t) {
         const int it = t - tile_beg, stage = it & 1;
-        const int nc = a.tiles[t].n_slots;
+        const TileMeta tm = a.tiles[t];
+        const int nc = tm.n_slots;
         const BCell* __restrict__ tC = sC + stage * TILE;
 #pragma unroll
         for (int k = 0; k < BQT; ++k)
@@ -156,13 +172,39 @@ __global__ void __launch_bounds__(AMP_THREADS, 3) k_amp_batch(const BatchArgs a)
             double p = 0.0;
             if (MODE == 0) p = fma(c1, YZ.y, c0 * YZ.x);
             if (MODE == 1) p = c0 * YZ.x;
+            u64 phs[BQT];
+            if (REC) {
+                float cd, sd;
+                const int kd = __double2loint(fma(dq, MODE == 0 ? p : YZ.y, MAGIC));
+                if (!ACC) sincos_mufu(kd, cd, sd);
+                else if (a.sh) sincos_poly_half(kd, cd, sd);
+                else sincos_poly(kd, cd, sd);
+                phs[KB] = phasor<ACC>(MODE == 0 ? fma(gb, p, MAGIC) : fma(gb, YZ.y, p) + MAGIC);
+                if (!ACC) {
+                    const float two_cd = cd + cd;
+                    phs[KB + 1] = rotate(phs[KB], cd, sd);
+#pragma unroll
+                    for (int k = KB + 2; k < BQT; ++k) phs[k] = three_term(phs[k - 1], phs[k - 2], two_cd);
+#pragma unroll
+                    for (int k = KB - 1; k >= 0; --k) phs[k] = three_term(phs[k + 1], phs[k + 2], two_cd);
+                } else {
+#pragma unroll
+                    for (int k = KB + 1; k < BQT; ++k) phs[k] = rotate(phs[k - 1], cd, sd);
+#pragma unroll
+                    for (int k = KB - 1; k >= 0; --k) phs[k] = rotate(phs[k + 1], cd, -sd);
+                }
+            }
 #pragma unroll
             for (int k = 0; k < BQT; ++k) {
-                double m;
-                if (MODE == 0) m = fma(g[k], p, MAGIC);
-                else if (MODE == 1) m = fma(g[k], YZ.y, p) + MAGIC;
-                else m = fma(g[k], YZ.y, h[k] * YZ.x) + MAGIC;
-                const u64 ph = phasor<ACC>(m);
+                u64 ph;
+                if (REC) ph = phs[k];
+                else {
+                    double m;
+                    if (MODE == 0) m = fma(g[k], p, MAGIC);
+                    else if (MODE == 1) m = fma(g[k], YZ.y, p) + MAGIC;
+                    else m = fma(g[k], YZ.y, h[k] * YZ.x) + MAGIC;
+                    ph = phasor<ACC>(m);
+                }
                 acc[k][0] = ffma2(pack2(w0.x, w0.x), ph, acc[k][0]);
                 acc[k][1] = ffma2(pack2(w0.y, w0.y), ph, acc[k][1]);
                 acc[k][2] = ffma2(pack2(w0.z, w0.z), ph, acc[k][2]);
@@ -176,14 +218,14 @@ __global__ void __launch_bounds__(AMP_THREADS, 3) k_amp_batch(const BatchArgs a)
             }
         };
         if (!ACC) {
-#pragma unroll 4
+#pragma unroll (REC ? 2 : 4)
             for (int j = 0; j < nc; ++j) cell(j);
         } else {
 #pragma unroll
             for (int r = 0; r < 2 * BQT; ++r) nacc[r * AMP_THREADS + tid] = 0.0;
             for (int j0 = 0; j0 < nc; j0 += NSUB_CELLS) {
                 const int j1 = min(nc, j0 + NSUB_CELLS);
-#pragma unroll 4
+#pragma unroll (REC ? 2 : 4)
                 for (int j = j0; j < j1; ++j) cell(j);
 #pragma unroll
                 for (int k = 0; k < BQT; ++k) {
@@ -197,16 +239,28 @@ __global__ void __launch_bounds__(AMP_THREADS, 3) k_amp_batch(const BatchArgs a)
         }
         __syncthreads();
         if (tid == 0 && t + 2 < tile_end) issue(t + 2, sC + stage * TILE, &bar[stage]);
+        double p0 = 0.0;                                   // projection of the tile centre (recurrence correction)
+        if (REC) p0 = MODE == 0 ? fma(c1, tm.Z0, c0 * tm.Y0) : tm.Z0;
 #pragma unroll
         for (int k = 0; k < BQT; ++k) {
             if (k < kmax) {
                 const int64_t f = flat0 + (int64_t)k * a.n1;
+                float eps = 0.f;
+                if (REC && k != KB) {
+                    const double gk = MODE == 0 ? (double)a.u0[i0 + k] * INV_2PI : a.qc[f].y * INV_2PI;
+                    eps = (float)(6.283185307179586 * (gk - (gb + (double)(k - KB) * dq)) * p0);
+                }
 #pragma unroll
                 for (int r = 0; r < BCH; ++r) {
                     float cs, sn;
                     unpack2(acc[k][r], cs, sn);
                     double dc = (double)cs, ds = (double)sn;
                     if (ACC && r == 0) { dc = nacc[(2 * k) * AMP_THREADS + tid]; ds = nacc[(2 * k + 1) * AMP_THREADS + tid]; }
+                    if (REC) {                             // cos(psi + eps), sin(psi + eps) to first order
+                        const double d2 = fma(-(double)eps, ds, dc);
+                        ds = fma((double)eps, dc, ds);
+                        dc = d2;
+                    }
                     atomicAdd(a.part + ((int64_t)chunk * 2 * BCH + 2 * r) * a.n_q + f, dc);        // Re: + sum w cos
                     atomicAdd(a.part + ((int64_t)chunk * 2 * BCH + 2 * r + 1) * a.n_q + f, -ds);   // Im: - sum w sin
                 }
@@ -254,15 +308,34 @@ nms_status launch_batch(nms_ctx* c, const float* m_batch, int B, const int32_t* 
 {
     if (nms_status st = wait_geometry(c)) return st;
     typedef void (*kern_t)(const BatchArgs);
-    kern_t kern = c->g_type == 0 ? (kern_t)k_amp_batch<0, false> : (c->g_type == 1 ? (kern_t)k_amp_batch<1, false> : (kern_t)k_amp_batch<2, false>);
-    if (accurate)
-        kern = c->g_type == 0 ? (kern_t)k_amp_batch<0, true> : (c->g_type == 1 ? (kern_t)k_amp_batch<1, true> : (kern_t)k_amp_batch<2, true>);
-    const size_t smem = BATCH_SMEM + (accurate ? (size_t)BQT * 2 * AMP_THREADS * sizeof(double) : 0);
+    // line recurrence: the ACCURATE variant where the lines are equally spaced and the cell order is spatially coherent (the
+    // criterion of plan_amplitude) -- its polynomial phasors cost FMA-pipe cycles, so one per 8 points pays (measured, 6
+    // fields: C5 2.12 -> 2.51, C4 geometry 2.19 -> 2.77 T pair-fields/s); the FAST variant stays direct (MUFU phasors run on
+    // the otherwise idle XU pipe: 2.99 direct against 2.81 with the recurrence on C5).  "variant" 1 forces the direct
+    // kernel, 2 the recurrence
+    const bool line_ok = c->g_type != 2 && c->g_uniform && c->g_n0 >= 2;
+    if (c->opt_variant == 2 && !line_ok)
+        return fail(c, NMS_E_UNSUPPORTED, "the line-recurrence variant needs a polar or Cartesian detector with equally spaced u0");
+    const bool rec = line_ok && (c->opt_variant == 2 || (c->opt_variant == 0 && accurate &&
+                                                         c->g_dev * (c->g_type == 0 ? c->geo_ext : c->geo_extz) <= 1e-4));
+    const int qt = rec ? BQT_REC : BQT;
+    kern_t kern;
+    if (rec) {
+        if (accurate) kern = c->g_type == 0 ? (kern_t)k_amp_batch<0, true, BQT_REC, true> : (kern_t)k_amp_batch<1, true, BQT_REC, true>;
+        else kern = c->g_type == 0 ? (kern_t)k_amp_batch<0, false, BQT_REC, true> : (kern_t)k_amp_batch<1, false, BQT_REC, true>;
+    } else if (accurate) {
+        kern = c->g_type == 0 ? (kern_t)k_amp_batch<0, true, BQT, false>
+                              : (c->g_type == 1 ? (kern_t)k_amp_batch<1, true, BQT, false> : (kern_t)k_amp_batch<2, true, BQT, false>);
+    } else {
+        kern = c->g_type == 0 ? (kern_t)k_amp_batch<0, false, BQT, false>
+                              : (c->g_type == 1 ? (kern_t)k_amp_batch<1, false, BQT, false> : (kern_t)k_amp_batch<2, false, BQT, false>);
+    }
+    const size_t smem = BATCH_SMEM + (accurate ? (size_t)qt * 2 * AMP_THREADS * sizeof(double) : 0);
     NMS_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int occ = 0;
     NMS_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, AMP_THREADS, smem));
     if (occ < 1) return fail(c, NMS_E_CUDA, "batch amplitude kernel does not fit on an SM");
-    const int64_t n_qb = (((int64_t)(c->g_n0 + BQT - 1) / BQT) * c->g_n1 + AMP_THREADS - 1) / AMP_THREADS;
+    const int64_t n_qb = (((int64_t)(c->g_n0 + qt - 1) / qt) * c->g_n1 + AMP_THREADS - 1) / AMP_THREADS;
     const int n_chunks = choose_chunks(c, n_qb, (int64_t)c->sm_count * occ, c->n_tiles, 8.0 * 2 * BCH * (double)c->n_q, 8, 2.0e9);
     const size_t part_bytes = sizeof(double) * 2 * BCH * (size_t)c->n_q * n_chunks;
     if (nms_status st = ensure(c, c->part, part_bytes)) return st;
@@ -285,6 +358,7 @@ nms_status launch_batch(nms_ctx* c, const float* m_batch, int B, const int32_t* 
     a.n_tiles = (int)c->n_tiles;
     a.type = c->g_type; a.n0 = c->g_n0; a.n1 = c->g_n1; a.n_q = c->n_q;
     a.u0 = (const float*)c->u0.p; a.qc = (const double2*)c->qc.p; a.sc = (const double2*)c->sc.p;
+    a.dq = c->g_dq; a.sh = fabs(c->g_dq) * c->geo_rmax < 0.24 * 6.283185307179586 ? 1 : 0;
     a.part = (double*)c->part.p;
     RespParams rp;
     rp.Px = c->P[0]; rp.Py = c->P[1]; rp.Pz = c->P[2]; rp.sN = c->sN; rp.sM = c->sM; rp.invV = c->invV;
@@ -306,8 +380,8 @@ nms_status launch_batch(nms_ctx* c, const float* m_batch, int B, const int32_t* 
         c->launches += 3;
         NMS_CUDA(c, cudaGetLastError());
     }
-    c->n_chunks_used = n_chunks; c->blocks_per_sm_used = occ; c->qt_used = BQT; c->variant_used = 16;
-    c->npoly_used = accurate ? BQT : 0; c->nb_used = 0; c->rec3_used = 0;
+    c->n_chunks_used = n_chunks; c->blocks_per_sm_used = occ; c->qt_used = qt; c->variant_used = rec ? 17 : 16;
+    c->npoly_used = accurate ? (rec ? 1 : qt) : 0; c->nb_used = rec ? 1 : 0; c->rec3_used = rec && !accurate ? 1 : 0;
     return NMS_OK;
 }
 
