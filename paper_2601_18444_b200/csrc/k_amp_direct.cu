@@ -2,6 +2,9 @@
 // by MUFU (NPOLY = 0) or by polynomial on the FMA and ALU pipes (NPOLY = QT: the accurate variant).  Moving only one
 // or two of a thread's eight phasors to the FMA pipe was measured SLOWER than all-MUFU on B200 (C3: 1820 -> 1448 /
 // 1351 Gpair/s): the polynomial phasor costs ~26 issue cycles against 6 + 16 XU cycles (profiles/r2_*.md).
+// 16 points per thread at 2 blocks per SM, which lifted the recurrence kernels, does not help here: the kernel is bound by
+// the XU pipe, not by per-line work (C3, per-particle split: 0.652 -> 0.564; with 2 / 3 / 4 of the 16 phasors by polynomial
+// 0.464 / 0.382 / 0.385).
 #include "k_amplitude.cuh"
 
 namespace nms {
