@@ -57,6 +57,7 @@ __global__ void __launch_bounds__(AMP_THREADS) k_amp_f64(const AmpArgs a)
 // (all with fp32 accumulation over a tile), 8 exact (fp64)
 static amp_kernel_t pick_kernel(const AmpPlan& p)
 {
+    if (p.interp) return amp_kernel_interp(p.variant == 3 ? 0 : 1);
     switch (p.variant) {
     case 1: return amp_kernel_direct(2, p.qt, p.split, p.nch, p.npoly, false);
     case 2: return amp_kernel_direct(0, p.qt, p.split, p.nch, p.npoly, p.uni);
@@ -181,22 +182,32 @@ nms_status plan_amplitude(nms_ctx* c, bool split, bool want_accurate, AmpPlan* p
     }
     p.uni = c->g_n1 % AMP_THREADS == 0 && c->opt_uniform != 1;
     p.sh = rec && accurate && fabs(c->g_dq) * c->geo_rmax < 0.24 * 6.283185307179586 && c->opt_uniform != 1;
+    // accurate variant, four channels, not split, default arrangement: generate every other point of a line and take the
+    // points in between from the sums (k_amp_interp.cu) -- admissible while the step phase of every cell stays within 0.2
+    // cycle (1 / (2 cos delta) <= 1.62) and the line has at least 3 points
+    p.interp = rec && accurate && !split && p.nch == 4 && p.qt == 16 && c->opt_interp != 1 && c->opt_uniform != 1 &&
+               c->g_n0 >= 3 && fabs(c->g_dq) * c->geo_rmax < 0.2 * 6.283185307179586;
+    if (c->opt_interp == 2 && !p.interp)
+        return fail(c, NMS_E_UNSUPPORTED, "the interpolating kernel needs the accurate four-channel line recurrence (not split, qt 0 / 16, "
+                                          "default bases / recurrence) and a step phase below 0.2 cycle (d r_max = %.3g cycles)",
+                    fabs(c->g_dq) * c->geo_rmax * INV_2PI);
     amp_kernel_t kern = pick_kernel(p);
     if (!kern) return fail(c, NMS_E_ARG, "no amplitude kernel for variant %d qt %d bases %d polynomial %d three-term %d",
                            p.variant, p.qt, p.nb, p.npoly, p.rec3);
-    const size_t smem = p.variant == 8 ? 0 : amp_smem_bytes(p.qt, p.nch, split, p.npoly != 0 && !split);
+    const size_t smem = p.variant == 8 ? 0 : p.interp ? AMP_SMEM_INTERP : amp_smem_bytes(p.qt, p.nch, split, p.npoly != 0 && !split);
     NMS_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int occ = 0;
     NMS_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, AMP_THREADS, smem));
     if (occ < 1) return fail(c, NMS_E_CUDA, "amplitude kernel does not fit on an SM");
     const int64_t slots = (int64_t)c->sm_count * occ;
     const int64_t n_qb = p.variant == 8 ? ceil_div(c->n_q, AMP_THREADS)
+                         : p.interp     ? ceil_div(ceil_div(c->g_n0 / 2 + 1, 8) * c->g_n1, AMP_THREADS)   // 8 primaries per thread
                                         : ceil_div(ceil_div(c->g_n0, p.qt) * c->g_n1, AMP_THREADS);
 
     // (per-particle split: capping the chunks so that the (8 + n_kinds) planes per chunk stay within 0.3 GB -- 46 chunks
     // instead of 148 on C3 -- was tried: DRAM writes 1.96 -> 1.66 GB only (the reductions of the object flushes, not the
     // footprint, make them), 1 % slower: not kept)
-    p.n_chunks = choose_chunks(c, n_qb, slots, units, 8.0 * (double)c->n_q * (split ? 8.0 + NMS_KIND_COUNT : 8.0), split ? 1 : 8, 2.0e9);
+    p.n_chunks = choose_chunks(c, n_qb, slots, units, 8.0 * (double)c->n_q * (split ? 8.0 + NMS_KIND_COUNT : p.interp ? 16.0 : 8.0), split ? 1 : 8, 2.0e9);
     p.n_qblocks = (int)n_qb; p.blocks_per_sm = occ;
     *plan = p;
     return NMS_OK;
@@ -230,6 +241,12 @@ nms_status launch_amplitude(nms_ctx* c, const AmpPlan& plan, const int32_t* kind
     const size_t form_bytes = sizeof(double) * (size_t)n_kinds * (size_t)c->n_q * n_chunks;
     if (nms_status st = ensure(c, c->part, part_bytes)) return st;
     if (plan.split) if (nms_status st = ensure(c, c->formpart, form_bytes)) return st;
+    const int n_prim = c->g_n0 / 2 + 1;   // interpolating kernel: even lines, and one beyond the edge when n0 is even
+    const size_t sb_bytes = sizeof(double) * 8 * (size_t)n_prim * (size_t)c->g_n1 * n_chunks;
+    if (plan.interp) {
+        if (nms_status st = ensure(c, c->interp_sb, sb_bytes)) return st;
+        if (nms_status st = ensure(c, c->interp_spb, sb_bytes)) return st;
+    }
     AmpArgs a;
     a.cells = (const Cell*)c->cells.p;
     a.tiles = (const TileMeta*)c->tile_meta.p;
@@ -238,23 +255,30 @@ nms_status launch_amplitude(nms_ctx* c, const AmpPlan& plan, const int32_t* kind
     a.type = c->g_type; a.n0 = c->g_n0; a.n1 = c->g_n1; a.n_q = c->n_q;
     a.u0 = (const float*)c->u0.p; a.dq = c->g_dq; a.qc = (const double2*)c->qc.p; a.sc = (const double2*)c->sc.p;
     a.part = (double*)c->part.p; a.form = (double*)c->formpart.p;
+    a.sb = (double*)c->interp_sb.p; a.spb = (double*)c->interp_spb.p; a.n_prim = n_prim;
     a.kinds = kinds_dev; a.n_kinds = n_kinds;
     a.rp.Px = c->P[0]; a.rp.Py = c->P[1]; a.rp.Pz = c->P[2]; a.rp.sN = c->sN; a.rp.sM = c->sM; a.rp.invV = c->invV;
 
     amp_kernel_t kern = pick_kernel(plan);
-    const size_t smem = plan.variant == 8 ? 0 : amp_smem_bytes(plan.qt, plan.nch, plan.split, plan.npoly != 0 && !plan.split);
+    const size_t smem = plan.variant == 8 ? 0 : plan.interp ? AMP_SMEM_INTERP : amp_smem_bytes(plan.qt, plan.nch, plan.split, plan.npoly != 0 && !plan.split);
     NMS_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     dim3 grid((unsigned)plan.n_qblocks, (unsigned)n_chunks);
     // the kernels accumulate into their chunk partials with reductions
     NMS_CUDA(c, cudaMemsetAsync(c->part.p, 0, part_bytes, c->stream));
     if (plan.split) NMS_CUDA(c, cudaMemsetAsync(c->formpart.p, 0, form_bytes, c->stream));
+    if (plan.interp) {
+        NMS_CUDA(c, cudaMemsetAsync(c->interp_sb.p, 0, sb_bytes, c->stream));
+        NMS_CUDA(c, cudaMemsetAsync(c->interp_spb.p, 0, sb_bytes, c->stream));
+    }
     if (nms_status st = timer_begin(c, c->amp_timer)) return st;
     kern<<<grid, AMP_THREADS, smem, c->stream>>>(a);
+    if (plan.interp) { launch_interp_combine(a, n_chunks, c->stream); c->launches += 1; }   // the odd lines, inside the timed region
     if (nms_status st = timer_end(c, c->amp_timer)) return st;
     c->launches += 1;
     NMS_CUDA(c, cudaGetLastError());
     c->variant_used = plan.variant; c->n_chunks_used = n_chunks; c->blocks_per_sm_used = plan.blocks_per_sm;
     c->qt_used = plan.qt; c->npoly_used = plan.npoly; c->nb_used = plan.nb; c->rec3_used = plan.rec3;
+    c->interp_used = plan.interp ? 1 : 0;
     return NMS_OK;
 }
 

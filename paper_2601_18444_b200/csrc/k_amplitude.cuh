@@ -63,6 +63,9 @@ struct AmpArgs {
     const double2* sc;   // (sin th, cos th)
     double* part;        // [n_chunks][8][n_q]
     double* form;        // split: [n_chunks][n_kinds][n_q]
+    double* sb;          // k_amp_interp: B sets of the primaries [n_chunks][8][n_prim * n1], plain ...
+    double* spb;         // ... and weighted with the projection of the tile centres
+    int n_prim;          // k_amp_interp: primaries (even lines, one more beyond the edge when n0 is even) per line
     const int32_t* kinds;
     int n_kinds;
     RespParams rp;
@@ -438,9 +441,16 @@ __global__ void __launch_bounds__(AMP_THREADS, MINB) k_amp(const AmpArgs a)
     }
 }
 
+// k_amp_interp: the sub-accumulators of both sets (as amp_smem_bytes(16, 4, false, true)) and the fp32 p_0-weighted B sums
+constexpr size_t AMP_SMEM_INTERP = amp_smem_bytes(16, 4, false, true) + (size_t)64 * AMP_THREADS * sizeof(float);
+
 // lookup functions of the three instantiation units (NULL if the combination is not built)
 amp_kernel_t amp_kernel_direct(int mode, int qt, bool split, int nch, int npoly, bool uni);
 amp_kernel_t amp_kernel_rec_polar(int qt, int nb, bool split, int nch, bool poly, bool rec3, bool uni, bool sh);
 amp_kernel_t amp_kernel_rec_cart(int qt, int nb, bool split, int nch, bool poly, bool rec3, bool uni, bool sh);
+// k_amp_interp.cu: the accurate variant that generates every other point of a line (mode 0 polar, 1 Cartesian), and the
+// pass that forms the points in between from the B sets
+amp_kernel_t amp_kernel_interp(int mode);
+void launch_interp_combine(const AmpArgs& a, int n_chunks, cudaStream_t stream);
 
 }  // namespace nms

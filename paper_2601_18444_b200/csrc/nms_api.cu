@@ -265,7 +265,7 @@ void nms_destroy(nms_ctx* c)
     DevBuf* bufs[] = {&c->raw_pos, &c->raw_N, &c->raw_m, &c->centres, &c->tile_src, &c->tile_meta, &c->cells,
                       &c->wsum, &c->u0, &c->u1, &c->qc, &c->sc, &c->amp64, &c->part, &c->formpart,
                       &c->chunk_begin, &c->kinds_dev, &c->bin_idx, &c->bin_sum, &c->bin_cnt, &c->modal_tab, &c->modal_ring,
-                      &c->tile_wsum, &c->qc_half, &c->sc_half, &c->diag, &c->batch_cells, &c->batch_ampN, &c->pix_cells, &c->pix_meta, &c->pix_u0, &c->pix_u1, &c->pix_qc, &c->pix_sc};
+                      &c->tile_wsum, &c->interp_sb, &c->interp_spb, &c->qc_half, &c->sc_half, &c->diag, &c->batch_cells, &c->batch_ampN, &c->pix_cells, &c->pix_meta, &c->pix_u0, &c->pix_u1, &c->pix_qc, &c->pix_sc};
     for (DevBuf* b : bufs) free_buf(*b);
     for (DevBuf& b : c->host_stage) free_buf(b);
     if (c->h_geo) cudaFreeHost(c->h_geo);
@@ -626,6 +626,7 @@ nms_status nms_set_option(nms_ctx* c, const char* key, int64_t value)
     else if (!strcmp(key, "friedel")) { if (value < 0 || value > 1) return fail(c, NMS_E_ARG, "friedel must be 0 or 1"); c->opt_friedel = (int)value; }
     else if (!strcmp(key, "uniform")) { c->opt_uniform = (int)value; }
     else if (!strcmp(key, "recurrence")) { if (value < 0 || value > 2) return fail(c, NMS_E_ARG, "recurrence must be 0, 1 or 2"); c->opt_rec3 = (int)value; }
+    else if (!strcmp(key, "interp")) { if (value < 0 || value > 2) return fail(c, NMS_E_ARG, "interp must be 0, 1 or 2"); c->opt_interp = (int)value; }
     else if (!strcmp(key, "qt")) { if (value != 0 && value != 4 && value != 8 && value != 16) return fail(c, NMS_E_ARG, "qt must be 0, 4, 8 or 16"); c->opt_qt = (int)value; }
     else return fail(c, NMS_E_ARG, "unknown option '%s'", key);
     return NMS_OK;
@@ -646,6 +647,7 @@ nms_status nms_get_info(nms_ctx* c, const char* key, int64_t* value)
     else if (!strcmp(key, "poly_phasors")) *value = c->npoly_used;
     else if (!strcmp(key, "bases")) *value = c->nb_used;
     else if (!strcmp(key, "three_term")) *value = c->rec3_used;
+    else if (!strcmp(key, "interp")) *value = c->interp_used;
     else if (!strcmp(key, "corr2d_variant")) *value = c->corr2d_variant;
     else return fail(c, NMS_E_ARG, "unknown info key '%s'", key);
     return NMS_OK;

@@ -68,10 +68,11 @@ struct nms_ctx {
     nms::DevBuf qc_half, sc_half;  // detector constants of the half rings
     int opt_uniform = 0;   // 1: never use the block-uniform instantiations (testing)
     int opt_rec3 = 0;      // recurrence kernels: 0 auto, 1 rotations, 2 three-term recurrence
+    int opt_interp = 0;    // accurate recurrence kernels: 0 auto (interpolating kernel where admissible), 1 never, 2 required
     int amp_timer = NMS_T_AMPLITUDE;   // timer class of the amplitude launch (-1: none, the caller times it)
     int64_t launches = 0;
     int variant_used = 0, n_chunks_used = 0, blocks_per_sm_used = 0, qt_used = 0;
-    int npoly_used = 0, nb_used = 0, rec3_used = 0, corr2d_variant = 0;
+    int npoly_used = 0, nb_used = 0, rec3_used = 0, corr2d_variant = 0, interp_used = 0;
 
     // sample (raw copy kept for nms_set_rotation)
     int64_t W = 0;
@@ -112,6 +113,7 @@ struct nms_ctx {
     bool amp_valid = false;
     nms::DevBuf amp64;                 // double [8][n_q]
     nms::DevBuf part, formpart;        // chunk partials
+    nms::DevBuf interp_sb, interp_spb; // k_amp_interp: chunk partials of the B sets (plain, and weighted with the tile centres)
     nms::DevBuf chunk_begin;           // int32 [n_chunks+1] (split mode only)
     std::vector<int32_t> h_chunk_begin;
     nms::DevBuf kinds_dev;             // int32 [<=13]
@@ -159,6 +161,7 @@ struct AmpPlan {
     int rec3;          // recurrence: three-term recurrence instead of rotations
     bool sh;           // accurate recurrence: the step phase stays within a quarter cycle (no quadrant logic)
     bool uni;          // n1 % 128 == 0: a block lies inside one group of lines (block-uniform abscissae)
+    bool interp;       // accurate recurrence: every other point of a line generated, the others interpolated (k_amp_interp.cu)
 };
 nms_status plan_amplitude(nms_ctx* c, bool split, bool want_accurate, AmpPlan* plan);
 int choose_chunks(nms_ctx* c, int64_t n_qb, int64_t slots, int64_t units, double chunk_bytes, int64_t min_units, double mem_bytes);

@@ -270,6 +270,60 @@ def test_recurrence_ragged_lines(nms, ctx, oracle_mod, gtype, n0, qt):
     report_signed_misses(misses)
 
 
+@pytest.mark.parametrize("gtype", [0, 1])
+@pytest.mark.parametrize("n0", [3, 4, 5, 15, 16, 17, 18, 33, 48])
+def test_interpolating_kernel_ragged_lines(nms, ctx, oracle_mod, gtype, n0):
+    """k_amp_interp (the accurate variant large problems get when the step phase of a line stays below 0.2 cycle):
+    every other point of a line is generated, the points in between are sums of their neighbours' h-weighted sets.
+    Lines of odd and even length (an even one needs one primary beyond the edge), shorter than, equal to and not a
+    multiple of the 16 points a thread covers, polar and Cartesian; amplitudes and all 13 kinds against the oracle.
+    A step phase beyond 0.2 cycle is refused when the kernel is required, and falls back when it is not."""
+    import torch
+    rng = np.random.Generator(np.random.Philox(4243))
+    W = 3000
+    pos = rng.uniform(-40, 40, size=(W, 3)).astype(np.float32)
+    N = rng.uniform(0.5, 1.5, size=W).astype(np.float32)
+    m = rng.normal(size=(W, 3)).astype(np.float32)
+    R = ni.rot_z(20.0) @ ni.rot_y(35.0) @ ni.rot_z(10.0)
+    u0 = 0.31 + 0.013 * np.arange(n0)                            # d r_max <= 0.013 * 69.3 = 0.9 rad = 0.14 cycle
+    if gtype == 0:
+        grid = ni.polar_grid(u0, 37)
+    else:
+        grid = ni.cartesian_grid(u0 - 0.5, np.linspace(-1.0, 1.0, 37))
+    kinds = list(ni.ALL_KINDS)
+    nms.nms_set_sample(ctx, _t(pos), _t(N), _t(m), R)
+    nms.nms_set_option(ctx, "variant", 2)
+    nms.nms_set_option(ctx, "qt", 16)
+    nms.nms_set_option(ctx, "precision", 2)
+    amp = torch.empty((8, grid.n_q), dtype=torch.float32, device="cuda")
+    maps = torch.empty((len(kinds), grid.n_q), dtype=torch.float32, device="cuda")
+    qy, qz, th = oracle_mod.grid_points(grid)
+    A, wsum = oracle_mod.amplitudes(pos, N, m, R, qy, qz, return_wsum=True)
+    M = oracle_mod.response(A, th, kinds)
+    misses = []
+    for interp in (2, 0, 1):                                     # required, automatic (= used), switched off
+        nms.nms_set_option(ctx, "interp", interp)
+        amp.fill_(float("nan")); maps.fill_(float("nan"))
+        nms.nms_amplitudes(ctx, grid, amp)
+        nms.nms_response(ctx, kinds, maps)
+        nms.nms_synchronize(ctx)
+        assert nms.nms_get_info(ctx, "variant_used") == (3 if gtype == 0 else 5)
+        assert nms.nms_get_info(ctx, "interp") == (0 if interp == 1 else 1)
+        assert nms.nms_get_info(ctx, "qt") == 16 and nms.nms_get_info(ctx, "poly_phasors") != 0
+        assert_amplitudes(amp.cpu().numpy(), A, wsum, f"interp {interp} n0={n0}")
+        assert_cross_sections(maps.cpu().numpy(), M, kinds, f"interp {interp} n0={n0}", signed_misses=misses)
+    coarse = ni.polar_grid(0.31 + 0.05 * np.arange(n0), 37) if gtype == 0 else \
+        ni.cartesian_grid(0.05 * np.arange(n0) - 0.2, np.linspace(-1.0, 1.0, 37))
+    nms.nms_set_option(ctx, "interp", 2)
+    with pytest.raises(nms.NmsError) as e:
+        nms.nms_amplitudes(ctx, coarse, None)
+    assert e.value.status == nms.NMS_E_UNSUPPORTED
+    nms.nms_set_option(ctx, "interp", 0)
+    nms.nms_amplitudes(ctx, coarse, None)
+    assert nms.nms_get_info(ctx, "interp") == 0
+    report_signed_misses(misses)
+
+
 # ---------------------------------------------------------------------------------------------------
 # C3, C4, C5 at BASELINE.json's full sizes, in the launch configuration bench.py times (automatic
 # variant): the full GPU map against the oracle on a seeded subset of detector points; maxima for the
@@ -319,21 +373,24 @@ def c5_full(oracle_mod):
     return wl, A, wsum, th
 
 
-@pytest.mark.parametrize("precision", [0, 1])
-def test_c5_full_map_end_to_end(nms, ctx, oracle_mod, c5_full, precision):
+@pytest.mark.parametrize("precision,interp", [(0, 0), (1, 0), (0, 1)])
+def test_c5_full_map_end_to_end(nms, ctx, oracle_mod, c5_full, precision, interp):
     """C5 at full size through the call sequence bench.py times (nms_compute, ring average, c(r), p(r)) against the
     FULL fp64 map of the oracle: all 13 maps at every one of the 262 144 detector points, the amplitudes, the 512-ring
     I(q) (Eq. 30) and c(r), p(r) at 1024 r (Eq. 34-35).
     precision 0: what the library picks itself for C5's 13 kinds -- the accurate variant (polynomial phasors, rotations,
-    fp64 sub-accumulation of the nuclear channel), the configuration of the headline bench line: every kind, NM and CHI
-    included, must meet the north_star criterion at every point.  precision 1: the fast variant (three-term recurrence,
-    MUFU phasors) forced: a miss of NM / CHI is reported as xfail."""
+    fp64 sub-accumulation of the nuclear channel; every other point of a line generated, the points in between taken from
+    the sums: k_amp_interp), the configuration of the headline bench line: every kind, NM and CHI included, must meet the
+    north_star criterion at every point -- and so must the accurate variant that generates all 16 points of a thread
+    (interp 1: the interpolating kernel switched off).  precision 1: the fast variant (three-term recurrence, MUFU
+    phasors) forced: a miss of NM / CHI is reported as xfail."""
     import torch
     wl, A, wsum, th = c5_full
     kinds = wl.kinds
     M = oracle_mod.response(A, th, kinds, P=wl.P)
     _upload(nms, ctx, wl)
     nms.nms_set_option(ctx, "precision", precision)
+    nms.nms_set_option(ctx, "interp", interp)
     nq, nb, nr, nk = wl.grid.n_q, wl.n_bins, len(wl.r), len(kinds)
     f32 = dict(dtype=torch.float32, device="cuda")
     maps, I, qb = torch.empty((nk, nq), **f32), torch.empty((nk, nb), **f32), torch.empty(nb, **f32)
@@ -347,6 +404,7 @@ def test_c5_full_map_end_to_end(nms, ctx, oracle_mod, c5_full, precision):
     nms.nms_synchronize(ctx)
     assert nms.nms_get_info(ctx, "variant_used") == 3
     assert (nms.nms_get_info(ctx, "poly_phasors") != 0) == (precision == 0)
+    assert nms.nms_get_info(ctx, "interp") == (1 if precision == 0 and interp == 0 else 0)
     np.testing.assert_allclose(nms.nms_get_weight_sums(ctx), wsum, rtol=1e-12)
     assert_amplitudes(amp.cpu().numpy(), A, wsum, "C5 full map")
     misses = [] if precision == 1 else None
