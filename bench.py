@@ -595,7 +595,7 @@ def measure(nms, torch, wl_full, args, steps, warmup, dist, rank, local_rank, wo
                 if clocks.get("sm_mhz") else None,
                 "variant": nms.nms_get_info(h, "variant_used"), "qt": nms.nms_get_info(h, "qt"),
                 "bases": nms.nms_get_info(h, "bases"), "three_term": nms.nms_get_info(h, "three_term"),
-                "poly_phasors": nms.nms_get_info(h, "poly_phasors"),
+                "poly_phasors": nms.nms_get_info(h, "poly_phasors"), "interpolating": nms.nms_get_info(h, "interp"),
                 "cell_chunks": nms.nms_get_info(h, "n_chunks"), "blocks_per_sm": nms.nms_get_info(h, "blocks_per_sm")}
     res = {"value": value, "ms_per_step": ms_step, "steps": steps, "warmup": warmup, "roofline": roofline,
            "clocks": clocks, "gpu_launches": launches, "pairs_per_step": wl_full.pairs}

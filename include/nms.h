@@ -289,6 +289,12 @@ NMS_API nms_status nms_get_weight_sums(nms_ctx* ctx, double* out);
  * (Eq. 42-43): half the pair evaluations; the second half then belongs to the float angle rotated by
  * its deviation from theta + pi (<= 2.4e-7 rad).  Off by default; bench.py reports it as an EFFECTIVE rate only.
  * "uniform": 1 = do not use the block-uniform instantiation of the polar recurrence kernel (testing).
+ * "interp": the accurate variant of the line-recurrence kernels (four channels, not split, 16 points per thread) generates
+ * only every other point of a line and takes the points in between from the sums -- the three-term identity
+ * z_{k-1} + z_{k+1} = 2 cos(delta) z_k read as an interpolation and applied, by the linearity of Eq. 42-47 (L353-L368), to
+ * h-weighted sums of the two neighbours (csrc/k_amp_interp.cu) -- wherever the step phase of every cell along the line
+ * stays below 0.2 cycle (d r_max < 0.4 pi).  0 automatic (used where admissible), 1 never, 2 required (NMS_E_UNSUPPORTED at
+ * compute time if it is not admissible).
  * Unknown keys: NMS_E_ARG.  The fp32 kernels need q_max r_max / 2 pi < 2^19 cycles (NMS_E_UNSUPPORTED
  * otherwise; the exact kernel has no such limit).                                                        */
 NMS_API nms_status nms_set_option(nms_ctx* ctx, const char* key, int64_t value);
@@ -296,7 +302,8 @@ NMS_API nms_status nms_set_option(nms_ctx* ctx, const char* key, int64_t value);
  * 2 polar direct, 4 cartesian direct, 3 polar recurrence, 5 cartesian recurrence, 8 exact fp64, 16 / 17 batched-field
  * kernel direct / line recurrence),
  * "n_chunks", "n_tiles", "n_slots", "sm_count", "blocks_per_sm", "qt", "poly_phasors" (non-zero: polynomial phasors),
- * "bases", "three_term", "corr2d_variant" (variant_used of the last nms_correlation_2d).             */
+ * "bases", "three_term", "interp" (1: the interpolating kernel ran), "corr2d_variant" (variant_used of the last
+ * nms_correlation_2d).                                                                              */
 NMS_API nms_status nms_get_info(nms_ctx* ctx, const char* key, int64_t* value);
 /* Device time in ms of the most recent launch of the given kernel class ("timing" must be 1);
  * synchronises on that kernel's end event.  NMS_E_STATE if it has not run.                       */
