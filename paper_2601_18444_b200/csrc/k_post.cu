@@ -286,7 +286,7 @@ nms_status launch_correlation_2d(nms_ctx* c, const float* map, const nms_qgrid* 
         int64_t n_tiles, n_slots, W, K, n_q;
         bool grid_valid, g_uniform, has_N, has_M, amp_valid;
         int g_type, g_n0, g_n1, opt_qt, opt_bases, amp_timer;
-        int variant_used, n_chunks_used, blocks_per_sm_used, qt_used, npoly_used, nb_used, rec3_used;
+        int variant_used, n_chunks_used, blocks_per_sm_used, qt_used, npoly_used, nb_used, rec3_used, interp_used;
         double g_dq, g_dev, g_qmax, geo_rmax, geo_ext, geo_extz;
         bool geo_pending;
         std::vector<float> h_u0, h_u1;
@@ -307,9 +307,9 @@ nms_status launch_correlation_2d(nms_ctx* c, const float* map, const nms_qgrid* 
         std::swap(sv.geo_ext, c->geo_ext); std::swap(sv.geo_extz, c->geo_extz); std::swap(sv.geo_pending, c->geo_pending);
     };
     auto keep_used = [&](bool save) {
-        int* u[] = {&c->variant_used, &c->n_chunks_used, &c->blocks_per_sm_used, &c->qt_used, &c->npoly_used, &c->nb_used, &c->rec3_used};
-        int* s[] = {&sv.variant_used, &sv.n_chunks_used, &sv.blocks_per_sm_used, &sv.qt_used, &sv.npoly_used, &sv.nb_used, &sv.rec3_used};
-        for (int i = 0; i < 7; ++i) { if (save) *s[i] = *u[i]; else *u[i] = *s[i]; }
+        int* u[] = {&c->variant_used, &c->n_chunks_used, &c->blocks_per_sm_used, &c->qt_used, &c->npoly_used, &c->nb_used, &c->rec3_used, &c->interp_used};
+        int* s[] = {&sv.variant_used, &sv.n_chunks_used, &sv.blocks_per_sm_used, &sv.qt_used, &sv.npoly_used, &sv.nb_used, &sv.rec3_used, &sv.interp_used};
+        for (int i = 0; i < 8; ++i) { if (save) *s[i] = *u[i]; else *u[i] = *s[i]; }
     };
     sv.cells = c->pix_cells; sv.tile_meta = c->pix_meta; sv.u0 = c->pix_u0; sv.u1 = c->pix_u1; sv.qc = c->pix_qc; sv.sc = c->pix_sc;
     sv.n_tiles = n_tiles; sv.n_slots = n_pix; sv.W = n_pix; sv.K = 0; sv.n_q = 0;
