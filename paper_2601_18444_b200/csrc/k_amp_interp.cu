@@ -17,8 +17,9 @@
 // primary itself) and with the weights h w (set B) -- and the odd points are the sums of their two neighbours' B sets.
 // Per 16 detector points: 64 packed accumulations as before, but 7 rotations instead of 15 and 8 live phasors instead
 // of 16 (13.4 -> 11.8 FMA-pipe cycles per pair).  The neighbour of a thread's last odd point belongs to another block, so
-// the B sets are flushed to their own chunk partials and k_interp_combine forms the odd points afterwards (per chunk, into
-// the same partials the other kernels fill: the epilogue is unchanged).  With an even number of lines the last line is odd
+// both sets are flushed to compact chunk partials indexed by primary and k_interp_combine writes the detector-shaped
+// partials afterwards (even lines: the A sets; odd lines: the sums of the neighbours' B sets; per chunk, the layout the other
+// kernels fill: the epilogue is unchanged).  With an even number of lines the last line is odd
 // and its upper neighbour is one more primary beyond the detector edge (the progression continues; only its B set is kept).
 //
 // Float-grid correction.  The kernel evaluates each thread's primaries on the exact progression a_k = g_b + 2 (k - k_b) d
@@ -176,8 +177,10 @@ __global__ void __launch_bounds__(AMP_THREADS, 2) k_amp_interp(const AmpArgs a)
         const double p0 = MODE == 0 ? fma(c1, tm.Z0, c0 * tm.Y0) : tm.Z0;
         const float p0f = (float)p0;
         const int64_t n_pq = (int64_t)a.n_prim * a.n1;
-        double* const pA = a.part + (int64_t)chunk * 8 * a.n_q + i1;   // + line n1 + plane n_q
-        double* const pS = a.sb + (int64_t)chunk * 8 * n_pq + i1;      // + primary n1 + plane n_pq
+        // both sets go to COMPACT partials indexed by primary ([chunk][A: 8 planes | B: 8 planes][n_prim n1]): writing the A
+        // sets straight into every other line of the detector-shaped partials made the L2 evict the lines under
+        // reduction nine times over (11 GB of DRAM writes per C5 launch against 0.6 GB with either set alone)
+        double* const pS = a.sb + (int64_t)chunk * 16 * n_pq + i1;     // + primary n1 + plane n_pq
 #pragma unroll
         for (int k = 0; k < QP; ++k) {
             const int pr = pr0 + k, line = 2 * pr;
@@ -194,18 +197,18 @@ __global__ void __launch_bounds__(AMP_THREADS, 2) k_amp_interp(const AmpArgs a)
                 unpack2(accB[k][w], cs, sn); B[2 * w] = (double)cs; B[2 * w + 1] = (double)sn;
             }
             if (line < a.n0) {   // set A: the amplitude at the primary, corrected to its float abscissa
-                double* q = pA + (int64_t)line * a.n1;
+                double* q = pS + (int64_t)pr * a.n1;
                 double eps = 0.0;
                 if (k != QP_B) eps = 6.283185307179586 * ((double)a.u0[line] * INV_2PI - (gb + (double)(2 * (k - QP_B)) * dq)) * p0;
 #pragma unroll
                 for (int w = 0; w < 4; ++w) {
                     const double cs = fma(-eps, A[2 * w + 1], A[2 * w]);          // cos(psi + eps), sin(psi + eps)
                     const double sn = fma(eps, A[2 * w], A[2 * w + 1]);
-                    atomicAdd(q, cs); q += a.n_q;        // Re: + sum w cos (Eq. 44, 46)
-                    atomicAdd(q, -sn); q += a.n_q;       // Im: - sum w sin (Eq. 45, 47)
+                    atomicAdd(q, cs); q += n_pq;         // Re: + sum w cos (Eq. 44, 46)
+                    atomicAdd(q, -sn); q += n_pq;        // Im: - sum w sin (Eq. 45, 47)
                 }
             }
-            double* q = pS + (int64_t)pr * a.n1;
+            double* q = pS + 8 * n_pq + (int64_t)pr * a.n1;
 #pragma unroll
             for (int w = 0; w < 4; ++w) {   // set B as (Re, Im) = (sum cos, - sum sin); times p_0: fp32 sums on chip
                 atomicAdd(q, B[2 * w]); q += n_pq;
@@ -231,28 +234,34 @@ __global__ void __launch_bounds__(AMP_THREADS, 2) k_amp_interp(const AmpArgs a)
     }
 }
 
-// Odd lines from the B sets of their two neighbouring primaries, per chunk, into the chunk partials.  A neighbour m
-// was evaluated at the abscissa a_m; the identity needs it at (float abscissa of the odd line) -/+ d: the difference
-// enters to first order through the p_0-weighted sums, (Re, Im) -> (Re + e Im, Im - e Re) summed over tiles with
-// e = 2 pi (difference) p_0 (the rule of the flush in k_amplitude.cuh, written for (Re, Im) = (sum cos, - sum sin)).
+// The detector-shaped chunk partials from the compact ones, per chunk: an even line is the A set of its primary; an odd
+// line is the sum of the B sets of its two neighbouring primaries.  A neighbour m was evaluated at the abscissa a_m; the
+// identity needs it at (float abscissa of the odd line) -/+ d: the difference enters to first order through the
+// p_0-weighted sums, (Re, Im) -> (Re + e Im, Im - e Re) summed over tiles with e = 2 pi (difference) p_0 (the rule of the
+// flush in k_amplitude.cuh, written for (Re, Im) = (sum cos, - sum sin)).
 __global__ void k_interp_combine(double* __restrict__ part, const double* __restrict__ sb, const double* __restrict__ spb,
                                  const float* __restrict__ u0, double dq_rad, int n0, int n1, int n_prim, int64_t n_q)
 {
-    const int n_odd = n0 / 2;
-    const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (idx >= (int64_t)n_odd * n1) return;
+    const int64_t f = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (f >= n_q) return;
     const int chunk = blockIdx.y;
-    const int m = (int)(idx / n1), i1 = (int)(idx % n1);
-    const int line = 2 * m + 1;
+    const int line = (int)(f / n1), i1 = (int)(f % n1);
+    const int64_t n_pq = (int64_t)n_prim * n1;
+    const int m = line >> 1;
+    const int64_t f_lo = (int64_t)m * n1 + i1, f_hi = f_lo + n1;
+    if (!(line & 1)) {
+        const double* sa = sb + (int64_t)chunk * 16 * n_pq + f_lo;
+#pragma unroll
+        for (int r = 0; r < 8; ++r) part[((int64_t)chunk * 8 + r) * n_q + f] = sa[r * n_pq];
+        return;
+    }
     const double dq = dq_rad * INV_2PI;
     const double gk = (double)u0[line] * INV_2PI;
     const double e_lo = 6.283185307179586 * ((gk - dq) - primary_abscissa(u0, n0, dq, m));
     const double e_hi = 6.283185307179586 * ((gk + dq) - primary_abscissa(u0, n0, dq, m + 1));
-    const int64_t n_pq = (int64_t)n_prim * n1;
-    const int64_t f_lo = (int64_t)m * n1 + i1, f_hi = f_lo + n1, f = (int64_t)line * n1 + i1;
 #pragma unroll
     for (int w = 0; w < 4; ++w) {
-        const double* sre = sb + ((int64_t)chunk * 8 + 2 * w) * n_pq;
+        const double* sre = sb + ((int64_t)chunk * 16 + 8 + 2 * w) * n_pq;
         const double* sim = sre + n_pq;
         const double* pre = spb + ((int64_t)chunk * 8 + 2 * w) * n_pq;
         const double* pim = pre + n_pq;
@@ -270,8 +279,7 @@ amp_kernel_t amp_kernel_interp(int mode)
 
 void launch_interp_combine(const AmpArgs& a, int n_chunks, cudaStream_t stream)
 {
-    const int64_t n = (int64_t)(a.n0 / 2) * a.n1;
-    if (n <= 0) return;
+    const int64_t n = a.n_q;
     dim3 grid((unsigned)((n + 255) / 256), (unsigned)n_chunks);
     k_interp_combine<<<grid, 256, 0, stream>>>(a.part, a.sb, a.spb, a.u0, a.dq, a.n0, a.n1, a.n_prim, a.n_q);
 }

@@ -207,7 +207,7 @@ nms_status plan_amplitude(nms_ctx* c, bool split, bool want_accurate, AmpPlan* p
     // (per-particle split: capping the chunks so that the (8 + n_kinds) planes per chunk stay within 0.3 GB -- 46 chunks
     // instead of 148 on C3 -- was tried: DRAM writes 1.96 -> 1.66 GB only (the reductions of the object flushes, not the
     // footprint, make them), 1 % slower: not kept)
-    p.n_chunks = choose_chunks(c, n_qb, slots, units, 8.0 * (double)c->n_q * (split ? 8.0 + NMS_KIND_COUNT : p.interp ? 16.0 : 8.0), split ? 1 : 8, 2.0e9);
+    p.n_chunks = choose_chunks(c, n_qb, slots, units, 8.0 * (double)c->n_q * (split ? 8.0 + NMS_KIND_COUNT : p.interp ? 20.0 : 8.0), split ? 1 : 8, 2.0e9);
     p.n_qblocks = (int)n_qb; p.blocks_per_sm = occ;
     *plan = p;
     return NMS_OK;
@@ -242,9 +242,9 @@ nms_status launch_amplitude(nms_ctx* c, const AmpPlan& plan, const int32_t* kind
     if (nms_status st = ensure(c, c->part, part_bytes)) return st;
     if (plan.split) if (nms_status st = ensure(c, c->formpart, form_bytes)) return st;
     const int n_prim = c->g_n0 / 2 + 1;   // interpolating kernel: even lines, and one beyond the edge when n0 is even
-    const size_t sb_bytes = sizeof(double) * 8 * (size_t)n_prim * (size_t)c->g_n1 * n_chunks;
+    const size_t sb_bytes = sizeof(double) * 8 * (size_t)n_prim * (size_t)c->g_n1 * n_chunks;   // 8 planes
     if (plan.interp) {
-        if (nms_status st = ensure(c, c->interp_sb, sb_bytes)) return st;
+        if (nms_status st = ensure(c, c->interp_sb, 2 * sb_bytes)) return st;    // A and B sets: 16 planes per chunk
         if (nms_status st = ensure(c, c->interp_spb, sb_bytes)) return st;
     }
     AmpArgs a;
@@ -264,10 +264,10 @@ nms_status launch_amplitude(nms_ctx* c, const AmpPlan& plan, const int32_t* kind
     NMS_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     dim3 grid((unsigned)plan.n_qblocks, (unsigned)n_chunks);
     // the kernels accumulate into their chunk partials with reductions
-    NMS_CUDA(c, cudaMemsetAsync(c->part.p, 0, part_bytes, c->stream));
+    if (!plan.interp) NMS_CUDA(c, cudaMemsetAsync(c->part.p, 0, part_bytes, c->stream));   // (interp: written by the combine pass)
     if (plan.split) NMS_CUDA(c, cudaMemsetAsync(c->formpart.p, 0, form_bytes, c->stream));
     if (plan.interp) {
-        NMS_CUDA(c, cudaMemsetAsync(c->interp_sb.p, 0, sb_bytes, c->stream));
+        NMS_CUDA(c, cudaMemsetAsync(c->interp_sb.p, 0, 2 * sb_bytes, c->stream));
         NMS_CUDA(c, cudaMemsetAsync(c->interp_spb.p, 0, sb_bytes, c->stream));
     }
     if (nms_status st = timer_begin(c, c->amp_timer)) return st;

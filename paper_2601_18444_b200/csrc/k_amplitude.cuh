@@ -63,8 +63,8 @@ struct AmpArgs {
     const double2* sc;   // (sin th, cos th)
     double* part;        // [n_chunks][8][n_q]
     double* form;        // split: [n_chunks][n_kinds][n_q]
-    double* sb;          // k_amp_interp: B sets of the primaries [n_chunks][8][n_prim * n1], plain ...
-    double* spb;         // ... and weighted with the projection of the tile centres
+    double* sb;          // k_amp_interp: A and B sets of the primaries [n_chunks][8 + 8][n_prim * n1] ...
+    double* spb;         // ... and the B sets weighted with the projection of the tile centres [n_chunks][8][n_prim * n1]
     int n_prim;          // k_amp_interp: primaries (even lines, one more beyond the edge when n0 is even) per line
     const int32_t* kinds;
     int n_kinds;
