@@ -274,7 +274,7 @@ NMS_API nms_status nms_get_weight_sums(nms_ctx* ctx, double* out);
  * kernel.  "precision": which variant of the fp32 kernels runs.  1 fast: MUFU phasors (sin.approx /
  * cos.approx on the exactly reduced phase), three-term recurrence; amplitudes and the positive kinds meet the north-star
  * tolerances, the signed difference kinds NM and CHI miss them at a fraction of a percent of their points.  2 accurate:
- * polynomial phasors to fp32 rounding, rotations, fp64 sub-accumulation of the nuclear channel; 25-30 % slower; meets the
+ * polynomial phasors to fp32 rounding, rotations, fp64 sub-accumulation of the nuclear channel; 20-30 % slower; meets the
  * tolerances for all 13 kinds on every config.  0 (default) automatic: accurate where NM / CHI may be formed from the sums
  * (nms_amplitudes, whose result nms_response and nms_cross_spectra use later; nms_compute, nms_form_factor_split and
  * nms_compute_batch when NMS_NM or NMS_CHI is among the kinds or amplitudes are returned), fast otherwise.
