@@ -940,6 +940,16 @@ def test_ragged_cell_counts(nms, ctx, oracle_mod, W):
         if qt:
             assert nms.nms_get_info(ctx, "qt") == qt
         assert_amplitudes(amp.cpu().numpy(), A, wsum, f"W={W} variant={variant} qt={qt} precision={prec}")
+    # the interpolating accurate kernel over the same ragged tiles (a finer |q| grid: its step phase must stay below 0.2 cycle)
+    fine = ni.polar_grid(0.3 + 0.02 * np.arange(19), 37)
+    qy, qz, th = oracle_mod.grid_points(fine)
+    A, wsum = oracle_mod.amplitudes(pos, N, m, None, qy, qz, return_wsum=True)
+    for key, value in (("variant", 2), ("qt", 16), ("precision", 2), ("interp", 2)):
+        nms.nms_set_option(ctx, key, value)
+    nms.nms_amplitudes(ctx, fine, amp)
+    nms.nms_synchronize(ctx)
+    assert nms.nms_get_info(ctx, "interp") == 1
+    assert_amplitudes(amp.cpu().numpy(), A, wsum, f"W={W} interpolating kernel")
 
 
 @pytest.mark.parametrize("variant,prec", [(0, 0), (1, 1), (1, 0)])
