@@ -144,9 +144,12 @@ __global__ void __launch_bounds__(AMP_THREADS, 2) k_amp_interp(const AmpArgs a)
                         u64 ph[QP];
                         ph[QP_B] = phasor<true>(MODE == 0 ? fma(gb, p, MAGIC) : fma(gb, YZ.y, p) + MAGIC);
 #pragma unroll
-                        for (int k = QP_B + 1; k < QP; ++k) ph[k] = rotate(ph[k - 1], c2, s2);
+                        for (int k = QP_B + 1; k < QP - 1; ++k) ph[k] = rotate(ph[k - 1], c2, s2);
 #pragma unroll
-                        for (int k = QP_B - 1; k >= 0; --k) ph[k] = rotate(ph[k + 1], c2, -s2);
+                        for (int k = QP_B - 1; k >= 1; --k) ph[k] = rotate(ph[k + 1], c2, -s2);
+                        // the two end points by ONE three-term step each (no chaining: the rounding of 2 cos enters once)
+                        ph[QP - 1] = three_term(ph[QP - 2], ph[QP - 3], c2 + c2);
+                        ph[0] = three_term(ph[1], ph[2], c2 + c2);
 #pragma unroll
                         for (int k = 0; k < QP; ++k) {
                             accumulate<4>(accA[k], w, ph[k]);
