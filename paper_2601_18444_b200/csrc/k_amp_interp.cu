@@ -12,11 +12,11 @@
 //
 //   A_c(q_k) = sum_j w_cj z_k^j = B_c(q_{k-1}) + B_c(q_{k+1}),   B_c(q_m) = sum_j (h_j w_cj) z_m^j.
 //
-// So a thread generates only the EVEN points of its line (its "primaries": one exactly evaluated polynomial phasor, 7
-// rotations by the doubled step) and accumulates each primary twice -- with the weights w (set A: the amplitude at the
+// So a thread generates only the EVEN points of its line (its "primaries": one exactly evaluated polynomial phasor, 4
+// rotations by the doubled step alternating with 3 single three-term steps) and accumulates each primary twice -- with the weights w (set A: the amplitude at the
 // primary itself) and with the weights h w (set B) -- and the odd points are the sums of their two neighbours' B sets.
-// Per 16 detector points: 64 packed accumulations as before, but 7 rotations instead of 15 and 8 live phasors instead
-// of 16 (13.4 -> 11.8 FMA-pipe cycles per pair).  The neighbour of a thread's last odd point belongs to another block, so
+// Per 16 detector points: 64 packed accumulations as before, but 4 rotations + 3 three-term steps instead of 15 rotations
+// and 8 live phasors instead of 16 (13.4 -> 11.5 FMA-pipe cycles per pair).  The neighbour of a thread's last odd point belongs to another block, so
 // both sets are flushed to compact chunk partials indexed by primary and k_interp_combine writes the detector-shaped
 // partials afterwards (even lines: the A sets; odd lines: the sums of the neighbours' B sets; per chunk, the layout the other
 // kernels fill: the epilogue is unchanged).  With an even number of lines the last line is odd
@@ -143,13 +143,17 @@ __global__ void __launch_bounds__(AMP_THREADS, 2) k_amp_interp(const AmpArgs a)
                         const float c2 = fmaf(-2.f * sd, sd, 1.f), s2 = 2.f * sd * cd;     // ... and of the doubled step
                         u64 ph[QP];
                         ph[QP_B] = phasor<true>(MODE == 0 ? fma(gb, p, MAGIC) : fma(gb, YZ.y, p) + MAGIC);
-#pragma unroll
-                        for (int k = QP_B + 1; k < QP - 1; ++k) ph[k] = rotate(ph[k - 1], c2, s2);
-#pragma unroll
-                        for (int k = QP_B - 1; k >= 1; --k) ph[k] = rotate(ph[k + 1], c2, -s2);
-                        // the two end points by ONE three-term step each (no chaining: the rounding of 2 cos enters once)
-                        ph[QP - 1] = three_term(ph[QP - 2], ph[QP - 3], c2 + c2);
-                        ph[0] = three_term(ph[1], ph[2], c2 + c2);
+                        // rotations alternate with SINGLE three-term steps z_{k+1} = 2 cos(2 delta) z_k - z_{k-1} (2 FFMA instead of 2 FMUL +
+                    // 2 FFMA): a step whose two inputs come from the base and a rotation adds the rounding of 2 cos once and is
+                    // not chained (two consecutive steps were measured: NM worst 9.8e-4 on the full C5 map against 6.5e-4 here)
+                        const float t2 = c2 + c2;
+                        ph[QP_B + 1] = rotate(ph[QP_B], c2, s2);
+                        ph[QP_B - 1] = rotate(ph[QP_B], c2, -s2);
+                        ph[QP_B + 2] = three_term(ph[QP_B + 1], ph[QP_B], t2);
+                        ph[QP_B - 2] = three_term(ph[QP_B - 1], ph[QP_B], t2);
+                        ph[QP_B + 3] = rotate(ph[QP_B + 2], c2, s2);
+                        ph[QP_B - 3] = rotate(ph[QP_B - 2], c2, -s2);
+                        ph[QP_B - 4] = three_term(ph[QP_B - 3], ph[QP_B - 2], t2);
 #pragma unroll
                         for (int k = 0; k < QP; ++k) {
                             accumulate<4>(accA[k], w, ph[k]);
