@@ -292,7 +292,8 @@ NMS_API nms_status nms_get_weight_sums(nms_ctx* ctx, double* out);
  * "interp": the accurate variant of the line-recurrence kernels (four channels, not split, 16 points per thread) generates
  * only every other point of a line and takes the points in between from the sums -- the three-term identity
  * z_{k-1} + z_{k+1} = 2 cos(delta) z_k read as an interpolation and applied, by the linearity of Eq. 42-47 (L353-L368), to
- * h-weighted sums of the two neighbours (csrc/k_amp_interp.cu) -- wherever the step phase of every cell along the line
+ * h-weighted sums of the two neighbours (csrc/k_amp_interp.cu; the generated points follow from one exactly evaluated
+ * point by rotations alternating with single, unchained three-term steps) -- wherever the step phase of every cell along the line
  * stays below 0.2 cycle (d r_max < 0.4 pi).  0 automatic (used where admissible), 1 never, 2 required (NMS_E_UNSUPPORTED at
  * compute time if it is not admissible).
  * Unknown keys: NMS_E_ARG.  The fp32 kernels need q_max r_max / 2 pi < 2^19 cycles (NMS_E_UNSUPPORTED
